@@ -1,0 +1,165 @@
+/* df_emul.h -- C-ABI boundary of libdfemul.so (NVIDIA B200, sm_100a only).
+ *
+ * The density-fitting (DF) Coulomb/exchange build of an SCF iteration with the
+ * two exchange contractions run as FP64 GEMMs emulated by INT8 tensor-core
+ * products (arXiv 2601.08077; citations are lines of the paper text PAPER.md).
+ *
+ *   rho_q  = sum_ij B^q_ij D_ij                PAPER.md:45   (Eq. 3)   FP64
+ *   J_ij   = sum_q  B^q_ij rho_q               PAPER.md:47   (Eq. 4)   FP64
+ *   X^q_ia = sum_j  B^q_ij C_ja                PAPER.md:49-51 (Eq. 5; blocked Eq. 12)  emulated
+ *   K_ij   = sum_q sum_a X^q_ia X^q_ja         PAPER.md:53   (Eq. 6; blocked Eq. 13) emulated
+ *
+ * Emulation ("fixed point ... Ozaki scheme", s = ceil((m_emu+1)/8)
+ * INT8 splits; s(s+1)/2 INT8 GEMMs).  Every detail the paper leaves
+ * open is fixed in DESIGN.md section 2 (readings R1..R13).
+ *
+ * Conventions for EVERY entry point
+ *  - All data pointers are DEVICE pointers to contiguous row-major arrays unless
+ *    the argument is documented as "host".  The caller owns every buffer; the
+ *    library only reads inputs, only writes outputs and its workspace, and keeps
+ *    no reference to caller memory after the call's work has run.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the default stream).
+ *    Work is enqueued on it; no entry point synchronises with the host unless it
+ *    says so.  Results are valid once the stream has reached the end of the call.
+ *  - Scratch memory comes from ONE caller-supplied workspace registered with
+ *    df_set_workspace(); one workspace serves one stream at a time.
+ *  - Return value: DF_OK (0) or a negative DF_ERR_* code.  No exceptions, no
+ *    printing.  Data-dependent faults (Inf/NaN, out-of-range magnitudes) do not
+ *    fail the call: they set bits in a device status word, see df_last_status().
+ *  - There is no CPU fallback: on a machine without an sm_100 device every
+ *    compute entry point returns DF_ERR_DEVICE.
+ */
+#ifndef DF_EMUL_H_
+#define DF_EMUL_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DF_OK             0
+#define DF_ERR_NULL      -1  /* a required pointer is NULL                    */
+#define DF_ERR_DIM       -2  /* a dimension is <= 0 or too large              */
+#define DF_ERR_TOL       -3  /* tol <= 0 or NaN, or slice count not in 1..8   */
+#define DF_ERR_WORKSPACE -4  /* no workspace registered, or it is too small   */
+#define DF_ERR_DEVICE    -5  /* no CUDA device of compute capability 10.x     */
+#define DF_ERR_CUDA      -6  /* a CUDA runtime / driver call failed           */
+#define DF_ERR_ALIGN     -7  /* a pointer is not 16-byte aligned              */
+
+#define DF_MODE_NOMINAL 0    /* tol -> s exactly as Table 1 */
+#define DF_MODE_GUARDED 1    /* one extra byte of margin (R7); default   */
+
+#define DF_STATUS_NONFINITE 1 /* an Inf/NaN was seen in an emulated operand   */
+#define DF_STATUS_RANGE     2 /* a row/column maximum outside [2^-450, 2^450] */
+
+/* ---- policy (host only, no device needed) ------------------------------- */
+
+/* Slice count s in 1..8 for a target relative Frobenius error `tol`
+ * (PAPER.md:130 s = ceil((m_emu+1)/8); R7).  mode = DF_MODE_*.
+ * Returns DF_ERR_TOL for tol <= 0 or NaN. */
+int df_slices_for_tol(double tol, int mode);
+
+/* Number of INT8 slice-pair products for s slices: s(s+1)/2. */
+int df_num_int8_gemms(int s);
+
+/* Largest contraction length accumulated in INT32 before a flush to FP64:
+ * 32*floor(131071/(32 s))  (R4). */
+int df_kflush(int s);
+
+/* Select the tol -> s mapping used by df_emul_gemm / df_jk_build. */
+int df_set_policy_mode(int mode);
+
+/* ---- workspace ---------------------------------------------------------- */
+
+/* Bytes of workspace df_emul_gemm needs for these sizes (s slices). */
+int64_t df_emul_gemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int s);
+
+/* Minimum bytes of workspace df_jk_build needs (s slices, naux processed in
+ * blocks of 512, BASELINE.json config 4).  A larger workspace lets the library
+ * batch several 512-blocks per launch. */
+int64_t df_jk_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, int s);
+
+/* Register a device buffer (256-byte aligned) as THE workspace.  The library
+ * never frees it.  Passing NULL/0 unregisters it. */
+int df_set_workspace(void* ptr, int64_t bytes);
+
+/* ---- the two mandated entry points -------------------------------------- */
+
+/* C = A . B emulated with s = df_slices_for_tol(tol) INT8 slices.
+ * A: m x k, B: k x n, C: m x n, all FP64 row-major, device.  C is overwritten.
+ * ||C_emul - A.B||_F / ||A.B||_F <= tol is the contract (guarded mode). */
+int df_emul_gemm(const double* A, const double* B, double* C,
+                 int64_t m, int64_t n, int64_t k, double tol, void* stream);
+
+/* One DF J/K build.
+ * B_packed: npair x naux FP64, npair = nao(nao+1)/2, q fastest, row
+ *           p = i(i+1)/2 + j holds B^q_ij for i >= j   (BASELINE.json config 0).
+ * C_occ: nao x nocc.  D: nao x nao, read as symmetric (0.5 (D + D^T)).
+ * J, K: nao x nao outputs, both triangles written, exactly symmetric.
+ * J is plain FP64; K = sum_q X^q X^q^T (no occupation factor,
+ * PAPER.md:53) is emulated with s = df_slices_for_tol(tol) in both GEMMs. */
+int df_jk_build(const double* B_packed, int64_t nao, int64_t naux,
+                const double* C_occ, int64_t nocc, const double* D,
+                double tol, double* J, double* K, void* stream);
+
+/* Same two calls with a forced slice count s in 1..8 (config 1's sweep). */
+int df_emul_gemm_slices(const double* A, const double* B, double* C,
+                        int64_t m, int64_t n, int64_t k, int s, void* stream);
+int df_jk_build_slices(const double* B_packed, int64_t nao, int64_t naux,
+                       const double* C_occ, int64_t nocc, const double* D,
+                       int s, double* J, double* K, void* stream);
+
+/* Copies the device status word (OR of DF_STATUS_* bits since the last call of
+ * this function) to *status (host) and clears it.  SYNCHRONISES `stream`. */
+int df_last_status(void* stream, int* status);
+
+/* ---- debug exports (tests only; not on the timed path) ------------------ */
+
+/* Row split (R2, steps 1-3): X is rows x cols FP64.  Writes
+ * e[rows] (int32 scale index) and planes[t][row][pitch] (int8, t = 0..s-1 is
+ * digit d_{t+1}); pitch = df_plane_pitch(cols); bytes past `cols` are zero. */
+int df_debug_split_rows(const double* X, int64_t rows, int64_t cols, int s,
+                        int32_t* e, int8_t* planes, void* stream);
+
+/* Column split of a k x n matrix: scale per column; planes[t][col][pitch]
+ * hold the TRANSPOSED digits (contraction index fastest), pitch = df_plane_pitch(k). */
+int df_debug_split_cols(const double* X, int64_t k, int64_t n, int s,
+                        int32_t* e, int8_t* planes, void* stream);
+
+/* Row pitch in bytes of a digit plane with `cols` contraction elements. */
+int64_t df_plane_pitch(int64_t cols);
+
+/* INT32 weight sums of one flush chunk, straight from TMEM:
+ * P[w-2][i][j] = sum_{t+u=w} sum_{kk in chunk} DA_t[i,kk] DB_u[j,kk], w = 2..s+1,
+ * chunk = [chunk*df_kflush(s), min(k, (chunk+1)*df_kflush(s))).
+ * DA: [s][m][pitch] int8, DB: [s][n][pitch] int8 (pitch = df_plane_pitch(k)).
+ * P: [s][m][n] int32.  With s = 1 this is one slice-pair product P^(1,1).
+ * bk selects the shared-memory swizzle / K-block width in bytes (32, 64, 128;
+ * 0 = the library's choice). */
+int df_debug_weight_sums(const int8_t* DA, const int8_t* DB,
+                         int64_t m, int64_t n, int64_t k, int s, int chunk,
+                         int bk, int32_t* P, void* stream);
+
+/* df_jk_build_slices that also exports GEMM(5)'s FP64 output
+ * X[i][q][a_pad] (a_pad = 16*ceil(nocc/16), padded columns are zero) and the
+ * GEMM(6) scale indices e6[g][i] of every q-group g (R5).  X_out /
+ * e6_out may be NULL.  *ngroups_out (host) receives the number of groups. */
+int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
+                      const double* C_occ, int64_t nocc, const double* D,
+                      int s, double* J, double* K,
+                      double* X_out, int32_t* e6_out, int* ngroups_out, void* stream);
+
+/* Number of GPU kernels this library has launched in this process. */
+int64_t df_launch_count(void);
+
+/* Back-to-back tcgen05.mma.kind::i8 issue-rate probe (operands resident in
+ * shared memory, no loads): runs `iters` MMAs of shape 128 x n_mma x 32 per CTA
+ * on every SM.  Returns the launch's device time in milliseconds in *ms (host);
+ * INT8 op/s = 2*128*n_mma*32*iters*grid / time.  Synchronises. */
+int df_debug_mma_peak(int n_mma, int iters, int grid, float* ms, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DF_EMUL_H_ */

@@ -1,0 +1,224 @@
+"""ctypes binding of libdfemul.so -- argument marshalling only (include/df_emul.h).
+
+Every function here has the name and argument order of the C entry point it calls;
+tensors are passed as `data_ptr()` and the stream as
+`torch.cuda.current_stream().cuda_stream`.  PyTorch is used for device memory and
+streams only.  Nothing is computed in Python and nothing falls back to the CPU: a
+missing library raises ImportError, a failing call raises DFError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+lib_path = os.path.join(_HERE, "libdfemul.so")
+
+if not os.path.exists(lib_path):
+    raise ImportError(
+        f"{lib_path} is missing: build it with `python -m paper_2601_08077_b200.build` "
+        "(there is no CPU fallback)"
+    )
+lib = C.CDLL(lib_path)
+
+DF_MODE_NOMINAL, DF_MODE_GUARDED = 0, 1
+DF_STATUS_NONFINITE, DF_STATUS_RANGE = 1, 2
+_ERRORS = {
+    -1: "DF_ERR_NULL", -2: "DF_ERR_DIM", -3: "DF_ERR_TOL", -4: "DF_ERR_WORKSPACE",
+    -5: "DF_ERR_DEVICE", -6: "DF_ERR_CUDA", -7: "DF_ERR_ALIGN",
+}
+
+
+class DFError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what} failed: {_ERRORS.get(code, code)}")
+        self.code = code
+
+
+_vp, _i64, _i32, _f64 = C.c_void_p, C.c_int64, C.c_int, C.c_double
+_SIG = {
+    "df_slices_for_tol": (_i32, [_f64, _i32]),
+    "df_num_int8_gemms": (_i32, [_i32]),
+    "df_kflush": (_i32, [_i32]),
+    "df_set_policy_mode": (_i32, [_i32]),
+    "df_plane_pitch": (_i64, [_i64]),
+    "df_emul_gemm_workspace_bytes": (_i64, [_i64, _i64, _i64, _i32]),
+    "df_jk_workspace_bytes": (_i64, [_i64, _i64, _i64, _i32]),
+    "df_set_workspace": (_i32, [_vp, _i64]),
+    "df_emul_gemm": (_i32, [_vp, _vp, _vp, _i64, _i64, _i64, _f64, _vp]),
+    "df_emul_gemm_slices": (_i32, [_vp, _vp, _vp, _i64, _i64, _i64, _i32, _vp]),
+    "df_jk_build": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _f64, _vp, _vp, _vp]),
+    "df_jk_build_slices": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
+    "df_last_status": (_i32, [_vp, C.POINTER(C.c_int)]),
+    "df_debug_split_rows": (_i32, [_vp, _i64, _i64, _i32, _vp, _vp, _vp]),
+    "df_debug_split_cols": (_i32, [_vp, _i64, _i64, _i32, _vp, _vp, _vp]),
+    "df_debug_weight_sums": (_i32, [_vp, _vp, _i64, _i64, _i64, _i32, _i32, _i32, _vp, _vp]),
+    "df_debug_jk_build": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp, _vp,
+                                 C.POINTER(C.c_int), _vp]),
+    "df_launch_count": (_i64, []),
+    "df_debug_mma_peak": (_i32, [_i32, _i32, _i32, C.POINTER(C.c_float), _vp]),
+}
+EXPORTS = tuple(_SIG)
+for _name, (_res, _args) in _SIG.items():
+    _fn = getattr(lib, _name)  # AttributeError if the library does not export it
+    _fn.restype, _fn.argtypes = _res, _args
+
+
+def _check(code: int, what: str) -> int:
+    if code < 0:
+        raise DFError(int(code), what)
+    return int(code)
+
+
+def _stream(stream=None):
+    if stream is not None:
+        return C.c_void_p(int(stream))
+    import torch
+
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t, dtype=None):
+    if t is None:
+        return C.c_void_p(0)
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"expected dtype {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+# ---- policy -------------------------------------------------------------------------------
+def df_slices_for_tol(tol: float, mode: int = DF_MODE_GUARDED) -> int:
+    return _check(lib.df_slices_for_tol(float(tol), int(mode)), "df_slices_for_tol")
+
+
+def df_num_int8_gemms(s: int) -> int:
+    return _check(lib.df_num_int8_gemms(int(s)), "df_num_int8_gemms")
+
+
+def df_kflush(s: int) -> int:
+    return _check(lib.df_kflush(int(s)), "df_kflush")
+
+
+def df_set_policy_mode(mode: int) -> None:
+    _check(lib.df_set_policy_mode(int(mode)), "df_set_policy_mode")
+
+
+def df_plane_pitch(cols: int) -> int:
+    return _check(lib.df_plane_pitch(int(cols)), "df_plane_pitch")
+
+
+# ---- workspace ----------------------------------------------------------------------------
+def df_emul_gemm_workspace_bytes(m: int, n: int, k: int, s: int) -> int:
+    return _check(lib.df_emul_gemm_workspace_bytes(m, n, k, s), "df_emul_gemm_workspace_bytes")
+
+
+def df_jk_workspace_bytes(nao: int, naux: int, nocc: int, s: int) -> int:
+    return _check(lib.df_jk_workspace_bytes(nao, naux, nocc, s), "df_jk_workspace_bytes")
+
+
+def df_set_workspace(buf) -> None:
+    """buf: a uint8 CUDA tensor (kept alive by the caller), or None to unregister."""
+    if buf is None:
+        _check(lib.df_set_workspace(None, 0), "df_set_workspace")
+    else:
+        _check(lib.df_set_workspace(_ptr(buf), buf.numel() * buf.element_size()), "df_set_workspace")
+
+
+class Workspace:
+    """Owns a device buffer and registers it as the library's workspace."""
+
+    def __init__(self, nbytes: int, device="cuda"):
+        import torch
+
+        self.buf = torch.empty(int(nbytes) + 256, dtype=torch.uint8, device=device)
+        off = (-self.buf.data_ptr()) % 256
+        self.view = self.buf[off: off + int(nbytes)]
+        df_set_workspace(self.view)
+
+    def close(self):
+        df_set_workspace(None)
+        self.buf = self.view = None
+
+
+# ---- the two entry points -----------------------------------------------------------------
+def df_emul_gemm(A, B, Cout, m, n, k, tol, stream=None) -> None:
+    import torch
+
+    _check(lib.df_emul_gemm(_ptr(A, torch.float64), _ptr(B, torch.float64), _ptr(Cout, torch.float64),
+                            m, n, k, float(tol), _stream(stream)), "df_emul_gemm")
+
+
+def df_emul_gemm_slices(A, B, Cout, m, n, k, s, stream=None) -> None:
+    import torch
+
+    _check(lib.df_emul_gemm_slices(_ptr(A, torch.float64), _ptr(B, torch.float64), _ptr(Cout, torch.float64),
+                                   m, n, k, int(s), _stream(stream)), "df_emul_gemm_slices")
+
+
+def df_jk_build(B_packed, nao, naux, C_occ, nocc, D, tol, J, K, stream=None) -> None:
+    import torch
+
+    f = torch.float64
+    _check(lib.df_jk_build(_ptr(B_packed, f), nao, naux, _ptr(C_occ, f), nocc, _ptr(D, f), float(tol),
+                           _ptr(J, f), _ptr(K, f), _stream(stream)), "df_jk_build")
+
+
+def df_jk_build_slices(B_packed, nao, naux, C_occ, nocc, D, s, J, K, stream=None) -> None:
+    import torch
+
+    f = torch.float64
+    _check(lib.df_jk_build_slices(_ptr(B_packed, f), nao, naux, _ptr(C_occ, f), nocc, _ptr(D, f), int(s),
+                                  _ptr(J, f), _ptr(K, f), _stream(stream)), "df_jk_build_slices")
+
+
+def df_last_status(stream=None) -> int:
+    out = C.c_int(0)
+    _check(lib.df_last_status(_stream(stream), C.byref(out)), "df_last_status")
+    return int(out.value)
+
+
+# ---- debug exports ------------------------------------------------------------------------
+def df_debug_split_rows(X, rows, cols, s, e, planes, stream=None) -> None:
+    import torch
+
+    _check(lib.df_debug_split_rows(_ptr(X, torch.float64), rows, cols, int(s), _ptr(e, torch.int32),
+                                   _ptr(planes, torch.int8), _stream(stream)), "df_debug_split_rows")
+
+
+def df_debug_split_cols(X, k, n, s, e, planes, stream=None) -> None:
+    import torch
+
+    _check(lib.df_debug_split_cols(_ptr(X, torch.float64), k, n, int(s), _ptr(e, torch.int32),
+                                   _ptr(planes, torch.int8), _stream(stream)), "df_debug_split_cols")
+
+
+def df_debug_weight_sums(DA, DB, m, n, k, s, chunk, bk, P, stream=None) -> None:
+    import torch
+
+    _check(lib.df_debug_weight_sums(_ptr(DA, torch.int8), _ptr(DB, torch.int8), m, n, k, int(s), int(chunk),
+                                    int(bk), _ptr(P, torch.int32), _stream(stream)), "df_debug_weight_sums")
+
+
+def df_debug_jk_build(B_packed, nao, naux, C_occ, nocc, D, s, J, K, X_out=None, e6_out=None, stream=None) -> int:
+    import torch
+
+    f = torch.float64
+    ng = C.c_int(0)
+    _check(lib.df_debug_jk_build(_ptr(B_packed, f), nao, naux, _ptr(C_occ, f), nocc, _ptr(D, f), int(s),
+                                 _ptr(J, f), _ptr(K, f), _ptr(X_out, f) if X_out is not None else None,
+                                 _ptr(e6_out, torch.int32) if e6_out is not None else None,
+                                 C.byref(ng), _stream(stream)), "df_debug_jk_build")
+    return int(ng.value)
+
+
+def df_launch_count() -> int:
+    return int(lib.df_launch_count())
+
+
+def df_debug_mma_peak(n_mma: int, iters: int, grid: int, stream=None) -> float:
+    ms = C.c_float(0.0)
+    _check(lib.df_debug_mma_peak(int(n_mma), int(iters), int(grid), C.byref(ms), _stream(stream)),
+           "df_debug_mma_peak")
+    return float(ms.value)

@@ -1,0 +1,482 @@
+// api.cu -- the C-ABI of libdfemul.so (include/df_emul.h): policy, workspace carving and the
+// launch sequences of df_emul_gemm and df_jk_build.  Host logic only; every step of the path
+// runs in the kernels of split.cu, gemm_i8.cu and jk.cu.  No cuBLAS, no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include <atomic>
+
+#include "../../include/df_emul.h"
+#include "internal.h"
+
+namespace dfe {
+
+static std::atomic<long long> g_launches{0};
+void count_launch(int n) { g_launches += n; }
+
+static void* g_ws = nullptr;
+static int64_t g_ws_bytes = 0;
+static int g_mode = DF_MODE_GUARDED;
+static int g_device_ok = -1;
+
+static int device_ok() {
+  if (g_device_ok < 0) {
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+      cudaGetLastError();
+      return 0;  // not cached: a later call may find a device
+    }
+    g_device_ok = (prop.major == 10) ? 1 : 0;
+  }
+  return g_device_ok;
+}
+
+static int slices_for_tol(double tol, int mode) {
+  if (!(tol > 0.0) || isnan(tol)) return DF_ERR_TOL;
+  const double lg = log2(1.0 / tol);
+  int s;
+  if (mode == DF_MODE_NOMINAL) {
+    // m_emu = ceil(log2(1/tol) - 0.05); s = ceil((m_emu + 1) / 8)   (Table 1)
+    long long m_emu = (long long)ceil(lg - 0.05);
+    if (m_emu < 0) m_emu = 0;
+    s = (int)((m_emu + 1 + 7) / 8);
+  } else {
+    // one extra byte of margin (R7)
+    s = (int)ceil((lg + 7.0) / 8.0);
+  }
+  if (s < 1) s = 1;
+  if (s > kMaxSlices) s = kMaxSlices;
+  return s;
+}
+
+// bump allocator over the registered workspace, 256-byte granularity
+struct Carver {
+  char* base;
+  int64_t off = 0;
+  explicit Carver(void* b) : base((char*)b) {}
+  template <typename T>
+  T* take(int64_t count) {
+    T* p = (T*)(base ? base + off : nullptr);
+    off += round_up(count * (int64_t)sizeof(T), 256);
+    return p;
+  }
+};
+
+static inline int pad16(int64_t n) { return (int)round_up(n, 16); }
+
+// ---------------------------------------------------------------------------
+// df_emul_gemm
+// ---------------------------------------------------------------------------
+struct GemmWs {
+  int* status;
+  int32_t *eA, *eB;
+  uint32_t* cmax;
+  int8_t *pa, *pb;
+  int64_t pitch, bytes;
+};
+
+static GemmWs carve_gemm(void* base, int64_t m, int64_t n, int64_t k, int s) {
+  Carver c(base);
+  GemmWs w;
+  w.status = c.take<int>(64);
+  w.eA = c.take<int32_t>(m);
+  w.eB = c.take<int32_t>(n);
+  w.cmax = c.take<uint32_t>(n);
+  w.pitch = plane_pitch(k);
+  w.pa = c.take<int8_t>((int64_t)s * m * w.pitch);
+  w.pb = c.take<int8_t>((int64_t)s * n * w.pitch);
+  w.bytes = c.off;
+  return w;
+}
+
+static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, int s,
+                          cudaStream_t st) {
+  if (!A || !B || !C) return DF_ERR_NULL;
+  if (m <= 0 || n <= 0 || k <= 0 || k > (1ll << 30) || m > (1ll << 31) || n > (1ll << 31)) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  if (!device_ok()) return DF_ERR_DEVICE;
+  if (!g_ws) return DF_ERR_WORKSPACE;
+  GemmWs w = carve_gemm(g_ws, m, n, k, s);
+  if (w.bytes > g_ws_bytes) return DF_ERR_WORKSPACE;
+
+  if (launch_split_rows(A, m, k, k, s, w.eA, w.pa, w.pitch, m * w.pitch, w.status, st) != cudaSuccess)
+    return DF_ERR_CUDA;
+  if (launch_split_cols(B, k, n, s, w.cmax, w.eB, w.pb, w.pitch, n * w.pitch, w.status, st) != cudaSuccess)
+    return DF_ERR_CUDA;
+
+  GemmProblem g = {};
+  g.A = w.pa;
+  g.B = w.pb;
+  g.a_rows = m;
+  g.b_rows = n;
+  g.k = k;
+  g.a_pitch = g.b_pitch = w.pitch;
+  g.a_plane_stride = m * w.pitch;
+  g.b_plane_stride = n * w.pitch;
+  g.s = s;
+  g.n_tile = n > 128 ? 128 : pad16(n);
+  g.bk = 0;
+  g.nz = 1;
+  g.zk = nullptr;
+  g.eA = w.eA;
+  g.eB = w.eB;
+  g.mode = kEpiC;
+  g.C = C;
+  g.ldc = n;
+  if (launch_gemm_i8(g, st) != cudaSuccess) return DF_ERR_CUDA;
+  return DF_OK;
+}
+
+// ---------------------------------------------------------------------------
+// df_jk_build
+// ---------------------------------------------------------------------------
+constexpr int kQBlock = 512;  // BASELINE.json config 4: "naux blocks of 512"
+
+struct JkWs {
+  int* status;
+  double* rho;
+  uint32_t* emax5;
+  double* Jp;
+  uint32_t* cmaxC;
+  int32_t* eC;
+  int8_t* pc;
+  int32_t* e5;
+  int8_t* p5;
+  double* X;
+  int *qgroup, *gcol;
+  uint32_t* xmax;
+  int32_t* e6;
+  int8_t* p6;
+  double* Kpart;
+  int64_t pitchj, pitch6, bytes;
+  int a_pad, QG, gpb, ngmax;
+};
+
+// QS = q per super-block (a multiple of 512, or naux when naux < 512)
+static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s, int64_t QS) {
+  Carver c(base);
+  JkWs w;
+  w.a_pad = pad16(nocc);
+  w.QG = kflush_for(s) / w.a_pad;
+  if (w.QG < 1) w.QG = 1;
+  w.gpb = (kQBlock + w.QG - 1) / w.QG;
+  w.ngmax = (int)((QS + kQBlock - 1) / kQBlock) * w.gpb;
+  w.pitchj = plane_pitch(nao);
+  w.pitch6 = plane_pitch(QS * w.a_pad);
+  w.status = c.take<int>(64);
+  w.rho = c.take<double>(naux);
+  w.emax5 = c.take<uint32_t>(nao * naux);
+  w.Jp = c.take<double>(nao * (nao + 1) / 2);
+  w.cmaxC = c.take<uint32_t>(w.a_pad);
+  w.eC = c.take<int32_t>(w.a_pad);
+  w.pc = c.take<int8_t>((int64_t)s * w.a_pad * w.pitchj);
+  w.e5 = c.take<int32_t>(QS * nao);
+  w.p5 = c.take<int8_t>((int64_t)s * QS * nao * w.pitchj);
+  w.X = c.take<double>(nao * QS * w.a_pad);
+  w.qgroup = c.take<int>(QS);
+  w.gcol = c.take<int>(w.ngmax + 1);
+  w.xmax = c.take<uint32_t>((int64_t)w.ngmax * nao);
+  w.e6 = c.take<int32_t>((int64_t)w.ngmax * nao);
+  w.p6 = c.take<int8_t>((int64_t)s * nao * w.pitch6);
+  w.Kpart = c.take<double>((int64_t)w.ngmax * nao * nao);
+  w.bytes = c.off;
+  return w;
+}
+
+// q-group tables of one super-block [qs0, qs1) (R5): q is cut into blocks of 512, every
+// block into runs of QG consecutive q.  qgroup[q - qs0] = local group id; gcol[g] = first X column
+// (= contraction offset of GEMM(6)) of group g; gcol[ng] = end.
+__global__ void jk_group_tables_kernel(int nq, int QG, int gpb, int a_pad, int ng, int* qgroup, int* gcol) {
+  for (int ql = threadIdx.x; ql < nq; ql += blockDim.x) qgroup[ql] = (ql / kQBlock) * gpb + (ql % kQBlock) / QG;
+  for (int g = threadIdx.x; g <= ng; g += blockDim.x) {
+    const int qstart = (g / gpb) * kQBlock + (g % gpb) * QG;
+    gcol[g] = (g == ng) ? nq * a_pad : qstart * a_pad;
+  }
+}
+
+static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Cocc, int64_t nocc, const double* D,
+                   int s, double* J, double* K, double* X_out, int32_t* e6_out, int* ngroups_out,
+                   cudaStream_t st) {
+  if (!Bp || !Cocc || !D || !J || !K) return DF_ERR_NULL;
+  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nao > 32768 || naux > (1 << 20)) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  if (!device_ok()) return DF_ERR_DEVICE;
+  if (!g_ws) return DF_ERR_WORKSPACE;
+  // largest super-block (multiple of 512 q, capped so that GEMM(6)'s contraction offsets and the
+  // row count of GEMM(5) stay in int32) that fits the workspace
+  int64_t QS = 0;
+  {
+    const int64_t nblk = (naux + kQBlock - 1) / kQBlock;
+    for (int64_t nb = nblk; nb >= 1; --nb) {
+      const int64_t qs = (nb == nblk) ? naux : nb * kQBlock;
+      if (qs * pad16(nocc) >= (1ll << 30) || qs * nao >= (1ll << 31) - 256) continue;
+      if (carve_jk(nullptr, nao, naux, nocc, s, qs).bytes <= g_ws_bytes) {
+        QS = qs;
+        break;
+      }
+    }
+  }
+  if (QS == 0) return DF_ERR_WORKSPACE;
+  JkWs w = carve_jk(g_ws, nao, naux, nocc, s, QS);
+  const int64_t npair = nao * (nao + 1) / 2;
+
+#define DFE_CK(x) \
+  if ((x) != cudaSuccess) return DF_ERR_CUDA;
+
+  // ---- J: rho (Eq. 3) fused with GEMM(5)'s row maxima, then J (Eq. 4) ----
+  DFE_CK(cudaMemsetAsync(w.rho, 0, sizeof(double) * naux, st));
+  DFE_CK(cudaMemsetAsync(w.emax5, 0, sizeof(uint32_t) * nao * naux, st));
+  DFE_CK(launch_jk_pass_a(Bp, (int)nao, (int)naux, D, w.rho, w.emax5, st));
+  DFE_CK(launch_jk_j_gemv(Bp, npair, (int)naux, w.rho, w.Jp, st));
+  DFE_CK(launch_jk_j_unpack(w.Jp, (int)nao, J, st));
+
+  // ---- right operand of GEMM(5): C_occ columns -> K-major planes, a_pad rows (padding rows 0) ----
+  DFE_CK(cudaMemsetAsync(w.eC, 0, sizeof(int32_t) * w.a_pad, st));
+  DFE_CK(cudaMemsetAsync(w.pc, 0, (size_t)s * w.a_pad * w.pitchj, st));
+  DFE_CK(launch_split_cols(Cocc, nao, nocc, s, w.cmaxC, w.eC, w.pc, w.pitchj, (int64_t)w.a_pad * w.pitchj,
+                           w.status, st));
+
+  int gtotal = 0;
+  for (int64_t qs0 = 0; qs0 < naux; qs0 += QS) {
+    const int64_t qs1 = qs0 + QS < naux ? qs0 + QS : naux;
+    const int nq = (int)(qs1 - qs0);
+    const int nfull = nq / kQBlock, rem = nq % kQBlock;
+    const int ng = nfull * w.gpb + (rem + w.QG - 1) / w.QG;
+    const int64_t ncol = (int64_t)nq * w.a_pad;
+    const int64_t pitch6 = plane_pitch(ncol);
+
+    jk_group_tables_kernel<<<1, 256, 0, st>>>(nq, w.QG, w.gpb, w.a_pad, ng, w.qgroup, w.gcol);
+    count_launch();
+    DFE_CK(cudaGetLastError());
+    DFE_CK(cudaMemsetAsync(w.xmax, 0, sizeof(uint32_t) * ng * nao, st));
+
+    // H2: unpack + split packed B -> planes5 rows (q, i), contraction j
+    DFE_CK(launch_jk_unpack_split(Bp, (int)nao, (int)naux, (int)qs0, (int)qs1, w.emax5, s, w.e5, w.p5, w.pitchj,
+                                  (int64_t)nq * nao * w.pitchj, w.status, st));
+    // GEMM(5): X[i][q][a] = sum_j B^q_ij C_ja   (Eq. 5 / Eq. 12)
+    GemmProblem g5 = {};
+    g5.A = w.p5;
+    g5.B = w.pc;
+    g5.a_rows = (int64_t)nq * nao;
+    g5.b_rows = w.a_pad;
+    g5.k = nao;
+    g5.a_pitch = g5.b_pitch = w.pitchj;
+    g5.a_plane_stride = (int64_t)nq * nao * w.pitchj;
+    g5.b_plane_stride = (int64_t)w.a_pad * w.pitchj;
+    g5.s = s;
+    g5.n_tile = w.a_pad;
+    g5.nz = 1;
+    g5.eA = w.e5;
+    g5.eB = w.eC;
+    g5.mode = kEpiX;
+    g5.C = w.X;
+    g5.nao = (int)nao;
+    g5.ldx = ncol;
+    g5.qgroup = w.qgroup;
+    g5.xmax = w.xmax;
+    DFE_CK(launch_gemm_i8(g5, st));
+    if (X_out)
+      DFE_CK(cudaMemcpy2DAsync(X_out + qs0 * w.a_pad, sizeof(double) * naux * w.a_pad, w.X, sizeof(double) * ncol,
+                               sizeof(double) * ncol, nao, cudaMemcpyDeviceToDevice, st));
+
+    // X -> planes6 with one scale per (i, group)
+    DFE_CK(launch_jk_split_x(w.X, (int)nao, ncol, ncol, s, ng, w.gcol, w.xmax, w.e6, w.p6, pitch6,
+                             (int64_t)nao * pitch6, w.status, st));
+    if (e6_out)
+      DFE_CK(cudaMemcpyAsync(e6_out + (int64_t)gtotal * nao, w.e6, sizeof(int32_t) * ng * nao,
+                             cudaMemcpyDeviceToDevice, st));
+
+    // GEMM(6): K_g = X_g X_g^T per group (Eq. 6 / Eq. 13), lower block triangle only
+    GemmProblem g6 = {};
+    g6.A = w.p6;
+    g6.B = w.p6;
+    g6.a_rows = g6.b_rows = nao;
+    g6.k = ncol;
+    g6.a_pitch = g6.b_pitch = pitch6;
+    g6.a_plane_stride = g6.b_plane_stride = (int64_t)nao * pitch6;
+    g6.s = s;
+    g6.n_tile = 128;
+    g6.nz = ng;
+    g6.zk = w.gcol;
+    g6.eA = w.e6;
+    g6.eB = w.e6;
+    g6.ea_stride = g6.eb_stride = nao;
+    g6.lower_only = 1;
+    g6.mode = kEpiC;
+    g6.C = w.Kpart;
+    g6.ldc = nao;
+    g6.c_stride = nao * nao;
+    DFE_CK(launch_gemm_i8(g6, st));
+    // H7: K += sum_g K_g in increasing-q order, mirrored to the upper triangle
+    DFE_CK(launch_jk_k_reduce(w.Kpart, ng, (int)nao, qs0 > 0 ? 1 : 0, K, st));
+    gtotal += ng;
+  }
+  if (ngroups_out) *ngroups_out = gtotal;
+#undef DFE_CK
+  return DF_OK;
+}
+
+}  // namespace dfe
+
+// ===========================================================================
+// extern "C" boundary
+// ===========================================================================
+using namespace dfe;
+
+extern "C" {
+
+int df_slices_for_tol(double tol, int mode) {
+  if (mode != DF_MODE_NOMINAL && mode != DF_MODE_GUARDED) return DF_ERR_TOL;
+  return slices_for_tol(tol, mode);
+}
+
+int df_num_int8_gemms(int s) { return (s < 1 || s > kMaxSlices) ? DF_ERR_TOL : s * (s + 1) / 2; }
+
+int df_kflush(int s) { return (s < 1 || s > kMaxSlices) ? DF_ERR_TOL : kflush_for(s); }
+
+int df_set_policy_mode(int mode) {
+  if (mode != DF_MODE_NOMINAL && mode != DF_MODE_GUARDED) return DF_ERR_TOL;
+  g_mode = mode;
+  return DF_OK;
+}
+
+int64_t df_plane_pitch(int64_t cols) { return cols <= 0 ? DF_ERR_DIM : plane_pitch(cols); }
+
+int64_t df_emul_gemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int s) {
+  if (m <= 0 || n <= 0 || k <= 0) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  return carve_gemm(nullptr, m, n, k, s).bytes;
+}
+
+int64_t df_jk_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, int s) {
+  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  const int64_t qs = naux < kQBlock ? naux : kQBlock;
+  return carve_jk(nullptr, nao, naux, nocc, s, qs).bytes;
+}
+
+int df_set_workspace(void* ptr, int64_t bytes) {
+  if (!ptr || bytes <= 0) {
+    g_ws = nullptr;
+    g_ws_bytes = 0;
+    return DF_OK;
+  }
+  if (((uintptr_t)ptr & 255) != 0) return DF_ERR_ALIGN;
+  if (bytes < 256) return DF_ERR_WORKSPACE;
+  if (!device_ok()) return DF_ERR_DEVICE;
+  if (cudaMemset(ptr, 0, 256) != cudaSuccess) return DF_ERR_CUDA;  // the status word
+  g_ws = ptr;
+  g_ws_bytes = bytes;
+  return DF_OK;
+}
+
+int df_emul_gemm(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, double tol,
+                 void* stream) {
+  const int s = slices_for_tol(tol, g_mode);
+  if (s < 0) return s;
+  return emul_gemm_impl(A, B, C, m, n, k, s, (cudaStream_t)stream);
+}
+
+int df_emul_gemm_slices(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, int s,
+                        void* stream) {
+  return emul_gemm_impl(A, B, C, m, n, k, s, (cudaStream_t)stream);
+}
+
+int df_jk_build(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
+                const double* D, double tol, double* J, double* K, void* stream) {
+  const int s = slices_for_tol(tol, g_mode);
+  if (s < 0) return s;
+  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+int df_jk_build_slices(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
+                       const double* D, int s, double* J, double* K, void* stream) {
+  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
+                      const double* D, int s, double* J, double* K, double* X_out, int32_t* e6_out,
+                      int* ngroups_out, void* stream) {
+  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, X_out, e6_out, ngroups_out, (cudaStream_t)stream);
+}
+
+int df_last_status(void* stream, int* status) {
+  if (!status) return DF_ERR_NULL;
+  if (!g_ws) return DF_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (cudaMemcpyAsync(status, g_ws, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return DF_ERR_CUDA;
+  if (cudaMemsetAsync(g_ws, 0, sizeof(int), st) != cudaSuccess) return DF_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return DF_ERR_CUDA;
+  return DF_OK;
+}
+
+int df_debug_split_rows(const double* X, int64_t rows, int64_t cols, int s, int32_t* e, int8_t* planes,
+                        void* stream) {
+  if (!X || !e || !planes) return DF_ERR_NULL;
+  if (rows <= 0 || cols <= 0) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  if (!device_ok()) return DF_ERR_DEVICE;
+  if (!g_ws) return DF_ERR_WORKSPACE;
+  const int64_t pitch = plane_pitch(cols);
+  if (launch_split_rows(X, rows, cols, cols, s, e, planes, pitch, rows * pitch, (int*)g_ws,
+                        (cudaStream_t)stream) != cudaSuccess)
+    return DF_ERR_CUDA;
+  return DF_OK;
+}
+
+int df_debug_split_cols(const double* X, int64_t k, int64_t n, int s, int32_t* e, int8_t* planes, void* stream) {
+  if (!X || !e || !planes) return DF_ERR_NULL;
+  if (k <= 0 || n <= 0) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  if (!device_ok()) return DF_ERR_DEVICE;
+  if (!g_ws || g_ws_bytes < 256 + round_up(4 * n, 256)) return DF_ERR_WORKSPACE;
+  const int64_t pitch = plane_pitch(k);
+  uint32_t* cmax = (uint32_t*)((char*)g_ws + 256);
+  if (launch_split_cols(X, k, n, s, cmax, e, planes, pitch, n * pitch, (int*)g_ws, (cudaStream_t)stream) !=
+      cudaSuccess)
+    return DF_ERR_CUDA;
+  return DF_OK;
+}
+
+int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t n, int64_t k, int s, int chunk,
+                         int bk, int32_t* P, void* stream) {
+  if (!DA || !DB || !P) return DF_ERR_NULL;
+  if (m <= 0 || n <= 0 || k <= 0 || k > (1ll << 30)) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  if (bk != 0 && bk != 32 && bk != 64 && bk != 128) return DF_ERR_DIM;
+  if (chunk < 0 || (int64_t)chunk * kflush_for(s) >= k) return DF_ERR_DIM;
+  if (!device_ok()) return DF_ERR_DEVICE;
+  const int64_t pitch = plane_pitch(k);
+  GemmProblem g = {};
+  g.A = DA;
+  g.B = DB;
+  g.a_rows = m;
+  g.b_rows = n;
+  g.k = k;
+  g.a_pitch = g.b_pitch = pitch;
+  g.a_plane_stride = m * pitch;
+  g.b_plane_stride = n * pitch;
+  g.s = s;
+  g.n_tile = n > 128 ? 128 : pad16(n);
+  g.bk = bk;
+  g.nz = 1;
+  g.mode = kEpiInt32;
+  g.P = P;
+  g.dbg_chunk = chunk;
+  if (launch_gemm_i8(g, (cudaStream_t)stream) != cudaSuccess) return DF_ERR_CUDA;
+  return DF_OK;
+}
+
+int64_t df_launch_count(void) { return (int64_t)g_launches.load(); }
+
+int df_debug_mma_peak(int n_mma, int iters, int grid, float* ms, void* stream) {
+  if (!ms) return DF_ERR_NULL;
+  if (n_mma < 16 || n_mma > 256 || (n_mma % 16) != 0 || iters < 2 || grid < 1) return DF_ERR_DIM;
+  if (!device_ok()) return DF_ERR_DEVICE;
+  if (launch_mma_peak(n_mma, iters, grid, ms, (cudaStream_t)stream) != cudaSuccess) return DF_ERR_CUDA;
+  return DF_OK;
+}
+
+}  // extern "C"

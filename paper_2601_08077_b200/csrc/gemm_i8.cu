@@ -1,0 +1,448 @@
+// gemm_i8.cu -- the INT8 slice-pair GEMM with fused FP64 recombination (rows H3, H4, H7 of
+// SURVEY.md section 8(a)); hand-written tcgen05.mma.kind::i8 for sm_100a.
+//
+// What one CTA computes (R3, R4, R6):
+//   for one 128 x n_tile output tile and one z item (a q-group, or the whole contraction),
+//   for each flush chunk of the contraction (<= kflush(s) elements, increasing k),
+//     for each pass (a run of at most W = 512 / n_tile weights, largest w first),
+//       P^(w) = sum_{t+u=w} D^A_t . D^B_u^T        -- INT32 accumulators in TMEM, one per weight
+//       out  += 2^(eA_i + eB_j + 2 - 8 w) P^(w)    -- w descending, ONE running FP64 sum
+//
+// Structure: warp 0 = TMA producer (one lane), warp 1 = TMEM allocator + MMA issuer (one lane),
+// warps 2..5 = epilogue (TMEM lane quarter = warp % 4).  All s digit planes of a K block sit in
+// shared memory together, so 2 s plane tiles feed up to s(s+1)/2 MMAs (hard
+// part 4).  Operands are K-major INT8 planes; the K-block width BK equals the TMA/UMMA swizzle
+// span (32, 64 or 128 bytes) and is chosen so that at least three stages fit.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "common.cuh"
+#include "internal.h"
+
+namespace dfe {
+
+constexpr int kMaxStages = 8;
+constexpr int kGemmThreads = 192;
+constexpr int kSmemLimit = 232448;  // 227 KB
+
+struct GemmKernelParams {
+  CUtensorMap mapA;
+  CUtensorMap mapB;
+  int s, n_tile, acc_stride, weights_per_pass;
+  int tiles_m, tiles_n, group_m;
+  int num_stages;
+  uint32_t stage_stride;
+  long long a_rows, b_rows;
+  int k;  // contraction extent
+  int kflush;
+  const int* zk;
+  const int32_t* eA;
+  const int32_t* eB;
+  long long ea_stride, eb_stride;
+  int lower_only, mode;
+  double* C;
+  long long ldc, c_stride;
+  int nao;
+  long long ldx;
+  const int* qgroup;
+  uint32_t* xmax;
+  int32_t* P;
+  int dbg_chunk;
+};
+
+// weights of pass `ps`: w_hi down to w_lo
+__device__ __forceinline__ void pass_weights(int s, int W, int ps, int& w_hi, int& w_lo) {
+  w_hi = s + 1 - ps * W;
+  w_lo = max(2, w_hi - W + 1);
+}
+
+template <int BK>
+__global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_constant__ GemmKernelParams p) {
+  // ---- tile coordinates (grouped rasterisation: bands of group_m tile rows) ----
+  int tm, tn;
+  {
+    const int lin = blockIdx.x;
+    const int per_band = p.group_m * p.tiles_n;
+    const int band = lin / per_band;
+    const int first_m = band * p.group_m;
+    const int gm = min(p.group_m, p.tiles_m - first_m);
+    const int r = lin - band * per_band;
+    tm = first_m + r % gm;
+    tn = r / gm;
+  }
+  if (p.lower_only && tn > tm) return;  // block-uniform, before any allocation
+  const int z = blockIdx.z;
+
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t full_bar[kMaxStages];
+  __shared__ __align__(8) uint64_t empty_bar[kMaxStages];
+  __shared__ __align__(8) uint64_t tmem_full_bar;
+  __shared__ __align__(8) uint64_t tmem_empty_bar;
+  __shared__ uint32_t tmem_slot;
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const int s = p.s;
+  const int W = p.weights_per_pass;
+  const int npass = (s + W - 1) / W;
+  const int S = p.num_stages;
+
+  // contraction range of this z item and its flush chunks
+  const int zk0 = p.zk ? p.zk[z] : 0;
+  const int zk1 = p.zk ? p.zk[z + 1] : p.k;
+  int chunk_lo = 0;
+  int chunk_hi = max(1, (zk1 - zk0 + p.kflush - 1) / p.kflush);
+  if (p.mode == kEpiInt32) {
+    chunk_lo = p.dbg_chunk;
+    chunk_hi = p.dbg_chunk + 1;
+  }
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tensormap(&p.mapA);
+    prefetch_tensormap(&p.mapB);
+    for (int i = 0; i < S; ++i) {
+      mbar_init(&full_bar[i], 1);
+      mbar_init(&empty_bar[i], 1);
+    }
+    mbar_init(&tmem_full_bar, 1);
+    mbar_init(&tmem_empty_bar, 128);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(&tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_slot;
+
+  const uint32_t a_plane_bytes = kTileM * BK;
+  const uint32_t b_plane_bytes = (uint32_t)p.n_tile * BK;
+  const uint32_t b_off = (uint32_t)s * a_plane_bytes;
+
+  if (warp == 0) {
+    // ================= TMA producer =================
+    if (lane == 0) {
+      uint32_t it = 0;
+      for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
+        const int kc0 = zk0 + ch * p.kflush;
+        const int kc1 = min(zk1, kc0 + p.kflush);
+        const int nkb = (kc1 - kc0 + BK - 1) / BK;
+        for (int ps = 0; ps < npass; ++ps) {
+          int w_hi, w_lo;
+          pass_weights(s, W, ps, w_hi, w_lo);
+          const int P = min(s, w_hi - 1);
+          const uint32_t tx = (uint32_t)P * (a_plane_bytes + b_plane_bytes);
+          for (int kb = 0; kb < nkb; ++kb, ++it) {
+            const uint32_t stage = it % S;
+            const uint32_t ph = (it / S) & 1u;
+            mbar_wait(&empty_bar[stage], ph ^ 1u);
+            uint8_t* st = smem + (size_t)stage * p.stage_stride;
+            mbar_expect_tx(&full_bar[stage], tx);
+            const int kpos = kc0 + kb * BK;
+            for (int t = 0; t < P; ++t)
+              tma_load_3d(st + t * a_plane_bytes, &p.mapA, &full_bar[stage], kpos, tm * kTileM, t);
+            for (int u = 0; u < P; ++u)
+              tma_load_3d(st + b_off + u * b_plane_bytes, &p.mapB, &full_bar[stage], kpos, tn * p.n_tile, u);
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ================= MMA issuer =================
+    if (lane == 0) {
+      const uint32_t idesc = make_idesc_i8(kTileM, p.n_tile);
+      uint32_t it = 0, iter = 0;
+      for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
+        const int kc0 = zk0 + ch * p.kflush;
+        const int kc1 = min(zk1, kc0 + p.kflush);
+        const int nkb = (kc1 - kc0 + BK - 1) / BK;
+        for (int ps = 0; ps < npass; ++ps, ++iter) {
+          int w_hi, w_lo;
+          pass_weights(s, W, ps, w_hi, w_lo);
+          if (iter > 0) {
+            mbar_wait(&tmem_empty_bar, (iter - 1) & 1u);
+            tc_fence_after();
+          }
+          for (int kb = 0; kb < nkb; ++kb, ++it) {
+            const uint32_t stage = it % S;
+            const uint32_t ph = (it / S) & 1u;
+            mbar_wait(&full_bar[stage], ph);
+            tc_fence_after();
+            const uint32_t sa = smem_u32(smem + (size_t)stage * p.stage_stride);
+            const int kpos = kc0 + kb * BK;
+            const int nkk = (min(BK, kc1 - kpos) + 31) / 32;
+            for (int kk = 0; kk < nkk; ++kk) {
+              for (int w = w_hi; w >= w_lo; --w) {
+                const int t_lo = max(1, w - s), t_hi = min(s, w - 1);
+                const uint32_t d_tmem = tmem_base + (uint32_t)((w_hi - w) * p.acc_stride);
+                for (int t = t_lo; t <= t_hi; ++t) {
+                  const int u = w - t;
+                  const uint64_t adesc = make_smem_desc(sa + (t - 1) * a_plane_bytes + kk * 32, BK);
+                  const uint64_t bdesc = make_smem_desc(sa + b_off + (u - 1) * b_plane_bytes + kk * 32, BK);
+                  const uint32_t acc = (kb > 0 || kk > 0 || t > t_lo) ? 1u : 0u;
+                  mma_i8_ss(d_tmem, adesc, bdesc, idesc, acc);
+                }
+              }
+            }
+            mma_commit(&empty_bar[stage]);  // frees the smem stage once these MMAs have read it
+          }
+          mma_commit(&tmem_full_bar);  // accumulators of this pass are complete
+        }
+      }
+    }
+  } else {
+    // ================= epilogue: TMEM -> FP64 recombination -> global =================
+    const int quarter = warp & 3;
+    const int row_local = quarter * 32 + lane;
+    const long long row = (long long)tm * kTileM + row_local;
+    const bool row_ok = row < p.a_rows;
+    const int eA = (row_ok && p.mode != kEpiInt32) ? p.eA[z * p.ea_stride + row] : 0;
+    const uint32_t t_lane = tmem_base + ((uint32_t)(quarter * 32) << 16);
+    const int col0 = tn * p.n_tile;
+
+    double* out = nullptr;
+    if (p.mode == kEpiC) {
+      out = p.C + z * p.c_stride + row * p.ldc;
+    } else if (p.mode == kEpiX) {
+      const long long q = row / p.nao;
+      const long long i = row - q * p.nao;
+      out = p.C + i * p.ldx + q * p.n_tile - col0;  // col0 == 0 in this mode
+    }
+    uint32_t iter = 0;
+    uint32_t hi_max = 0;
+    for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
+      for (int ps = 0; ps < npass; ++ps, ++iter) {
+        int w_hi, w_lo;
+        pass_weights(s, W, ps, w_hi, w_lo);
+        const bool first = (ch == chunk_lo) && (ps == 0);
+        const bool last = (ch == chunk_hi - 1) && (ps == npass - 1);
+        mbar_wait(&tmem_full_bar, iter & 1u);
+        tc_fence_after();
+        for (int c = 0; c < p.n_tile; c += 16) {
+          uint32_t v[16];
+          if (p.mode == kEpiInt32) {
+            for (int w = w_hi; w >= w_lo; --w) {
+              tmem_ld16(t_lane + (uint32_t)((w_hi - w) * p.acc_stride + c), v);
+              tmem_ld_wait();
+              if (row_ok) {
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                  const long long col = col0 + c + j;
+                  if (col < p.b_rows) p.P[((long long)(w - 2) * p.a_rows + row) * p.b_rows + col] = (int32_t)v[j];
+                }
+              }
+            }
+            continue;
+          }
+          double acc[16];
+          int eBv[16];
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            const long long col = col0 + c + j;
+            const bool ok = row_ok && col < p.b_rows;
+            eBv[j] = ok ? p.eB[z * p.eb_stride + col] : 0;
+            acc[j] = (ok && !first) ? out[col] : 0.0;
+          }
+          for (int w = w_hi; w >= w_lo; --w) {
+            tmem_ld16(t_lane + (uint32_t)((w_hi - w) * p.acc_stride + c), v);
+            tmem_ld_wait();
+            const int eb = eA + 2 - 8 * w;
+#pragma unroll
+            for (int j = 0; j < 16; ++j)
+              acc[j] = fma((double)(int32_t)v[j], pow2_double(eb + eBv[j]), acc[j]);
+          }
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            const long long col = col0 + c + j;
+            if (row_ok && col < p.b_rows) {
+              out[col] = acc[j];
+              if (last) hi_max = max(hi_max, abs_hi_word(acc[j]));
+            }
+          }
+        }
+        tc_fence_before();
+        mbar_arrive(&tmem_empty_bar);
+      }
+    }
+    if (p.mode == kEpiX && row_ok) {
+      const long long q = row / p.nao;
+      const long long i = row - q * p.nao;
+      atomicMax(&p.xmax[(long long)p.qgroup[q] * p.nao + i], hi_max);
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+// ---------------------------------------------------------------------------
+// tcgen05.mma.kind::i8 issue-rate probe: operands resident in shared memory, no loads.
+// MEASURED_PEAKS.json has no INT8 figure; this gives the roofline denominator.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(128, 1) mma_peak_kernel(int n_mma, int iters) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t done_bar;
+  __shared__ uint32_t tmem_slot;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // A: 128 rows x 32 B (SW32 tile, 4 KB), B: n_mma rows x 32 B, zero-filled
+  for (int i = threadIdx.x; i < (128 + 256) * 32 / 4; i += blockDim.x) ((uint32_t*)smem)[i] = 0;
+  if (threadIdx.x == 0) {
+    mbar_init(&done_bar, 1);
+    fence_barrier_init();
+  }
+  fence_proxy_async();
+  if (warp == 0) tmem_alloc(&tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_slot;
+  if (warp == 0 && lane == 0) {
+    const uint32_t idesc = make_idesc_i8(128, n_mma);
+    const uint64_t adesc = make_smem_desc(smem_u32(smem), 32);
+    const uint64_t bdesc = make_smem_desc(smem_u32(smem + 128 * 32), 32);
+    for (int i = 0; i < iters; ++i) mma_i8_ss(tmem_base + (uint32_t)((i & 1) * 256), adesc, bdesc, idesc, i > 1);
+    mma_commit(&done_bar);
+    mbar_wait(&done_bar, 0);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStream_t st) {
+  cudaError_t err = cudaFuncSetAttribute(mma_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384);
+  if (err != cudaSuccess) return err;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  mma_peak_kernel<<<grid, 128, 16384, st>>>(n_mma, 64);  // warm-up
+  cudaEventRecord(e0, st);
+  mma_peak_kernel<<<grid, 128, 16384, st>>>(n_mma, iters);
+  cudaEventRecord(e1, st);
+  count_launch(2);
+  err = cudaEventSynchronize(e1);
+  if (err == cudaSuccess) err = cudaEventElapsedTime(ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (err != cudaSuccess) return err;
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------
+// host side: tensor maps and launch
+// ---------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)ptr;
+  }
+  return fn;
+}
+
+// planes [plane][rows][pitch] int8 -> 3-D map (k, rows, plane), box (bk, box_rows, 1)
+static bool make_plane_map(CUtensorMap* map, const int8_t* base, int64_t k, int64_t rows, int planes,
+                           int64_t pitch, int64_t plane_stride, int bk, int box_rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[3] = {(cuuint64_t)k, (cuuint64_t)rows, (cuuint64_t)planes};
+  cuuint64_t strides[2] = {(cuuint64_t)pitch, (cuuint64_t)plane_stride};
+  cuuint32_t box[3] = {(cuuint32_t)bk, (cuuint32_t)box_rows, 1u};
+  cuuint32_t estr[3] = {1u, 1u, 1u};
+  const CUtensorMapSwizzle swz = bk == 128  ? CU_TENSOR_MAP_SWIZZLE_128B
+                                 : bk == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
+                                            : CU_TENSOR_MAP_SWIZZLE_32B;
+  CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void*)base, dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+static uint32_t stage_stride_for(int s, int n_tile, int bk) {
+  return (uint32_t)round_up((int64_t)s * (kTileM + n_tile) * bk, 1024);
+}
+
+cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
+  GemmKernelParams p;
+  const int s = g.s;
+  int bk = g.bk;
+  if (bk == 0) {
+    bk = 32;
+    for (int cand = 128; cand >= 32; cand /= 2)
+      if ((kSmemLimit - 2048) / (int)stage_stride_for(s, g.n_tile, cand) >= 3) {
+        bk = cand;
+        break;
+      }
+  }
+  p.stage_stride = stage_stride_for(s, g.n_tile, bk);
+  p.num_stages = (int)((kSmemLimit - 2048) / p.stage_stride);
+  if (p.num_stages > kMaxStages) p.num_stages = kMaxStages;
+  if (p.num_stages < 1) return cudaErrorInvalidValue;
+  if (!make_plane_map(&p.mapA, g.A, g.k, g.a_rows, s, g.a_pitch, g.a_plane_stride, bk, kTileM) ||
+      !make_plane_map(&p.mapB, g.B, g.k, g.b_rows, s, g.b_pitch, g.b_plane_stride, bk, g.n_tile))
+    return cudaErrorInvalidValue;
+  p.s = s;
+  p.n_tile = g.n_tile;
+  p.acc_stride = (int)round_up(g.n_tile, 32);
+  p.weights_per_pass = 512 / p.acc_stride;
+  if (p.weights_per_pass > s) p.weights_per_pass = s;
+  p.tiles_m = (int)((g.a_rows + kTileM - 1) / kTileM);
+  p.tiles_n = (int)((g.b_rows + g.n_tile - 1) / g.n_tile);
+  p.group_m = 16;
+  p.a_rows = g.a_rows;
+  p.b_rows = g.b_rows;
+  p.k = (int)g.k;
+  p.kflush = kflush_for(s);
+  p.zk = g.zk;
+  p.eA = g.eA;
+  p.eB = g.eB;
+  p.ea_stride = g.ea_stride;
+  p.eb_stride = g.eb_stride;
+  p.lower_only = g.lower_only;
+  p.mode = g.mode;
+  p.C = g.C;
+  p.ldc = g.ldc;
+  p.c_stride = g.c_stride;
+  p.nao = g.nao;
+  p.ldx = g.ldx;
+  p.qgroup = g.qgroup;
+  p.xmax = g.xmax;
+  p.P = g.P;
+  p.dbg_chunk = g.dbg_chunk;
+
+  const size_t smem = (size_t)p.num_stages * p.stage_stride + 1024;
+  dim3 grid((unsigned)((int64_t)p.tiles_m * p.tiles_n), 1, (unsigned)g.nz);
+  cudaError_t err;
+#define DFE_LAUNCH(BKV)                                                                                 \
+  err = cudaFuncSetAttribute(gemm_i8_kernel<BKV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+  if (err != cudaSuccess) return err;                                                                   \
+  gemm_i8_kernel<BKV><<<grid, kGemmThreads, smem, st>>>(p);
+  if (bk == 128) {
+    DFE_LAUNCH(128)
+  } else if (bk == 64) {
+    DFE_LAUNCH(64)
+  } else {
+    DFE_LAUNCH(32)
+  }
+#undef DFE_LAUNCH
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace dfe

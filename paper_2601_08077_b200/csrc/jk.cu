@@ -1,0 +1,288 @@
+// jk.cu -- the HBM-bound passes of df_jk_build around the two emulated GEMMs
+// (rows H1, H2, H5, H6, H7 of SURVEY.md section 8(a)).
+//
+//   jk_pass_a        rho_q = sum_ij B^q_ij D_ij (Eq. 3) fused with the row maxima
+//                    max_j |B^q_ij| that GEMM(5)'s left-operand scales need (R5)
+//   jk_j_gemv        J_p = sum_q B[p,q] rho_q   (Eq. 4), plain FP64
+//   jk_unpack_split  packed-symmetric B -> dense rows (q,i) x j as INT8 digit planes
+//                    ("symmetrise block to dense", fused with the split)
+//   jk_split_x       X (GEMM(5) output) -> digit planes with one scale per (i, q-group)
+//   jk_k_reduce      K = sum_g K_g in increasing-q order (Eq. 13), mirrored
+//
+// Geometry of the passes over packed B (q fastest): a block owns a 32 x 32 tile (rows R, columns
+// C) of the UNPACKED nao x nao matrix and 32 consecutive q; lane <-> q so every load is a 256-byte
+// run of one packed row p(max(R,C), min(R,C)).  Tile (a,b) and its mirror (b,a) read the same
+// packed rows; they get adjacent block indices so the second read is an L2 hit.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "common.cuh"
+#include "internal.h"
+
+namespace dfe {
+
+// block index -> (row tile TR, column tile TC) of the full square; returns false for the unused
+// mirror of a diagonal tile.
+__device__ __forceinline__ bool tile_of_block(unsigned bx, int& TR, int& TC, bool& lower) {
+  const unsigned idx = bx >> 1;
+  const int flip = bx & 1;
+  int a = (int)((sqrtf(8.0f * (float)idx + 1.0f) - 1.0f) * 0.5f);
+  while ((unsigned)(a + 1) * (unsigned)(a + 2) / 2 <= idx) ++a;
+  while ((unsigned)a * (unsigned)(a + 1) / 2 > idx) --a;
+  const int b = (int)(idx - (unsigned)a * (unsigned)(a + 1) / 2);
+  if (flip && a == b) return false;
+  TR = flip ? b : a;
+  TC = flip ? a : b;
+  lower = !flip;
+  return true;
+}
+
+__device__ __forceinline__ long long packed_row(int R, int C) {
+  const long long hi = max(R, C), lo = min(R, C);
+  return hi * (hi + 1) / 2 + lo;
+}
+
+__global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict__ Bp, int nao, int naux,
+                                                        const double* __restrict__ D, double* __restrict__ rho,
+                                                        uint32_t* __restrict__ emax) {
+  int TR, TC;
+  bool lower;
+  if (!tile_of_block(blockIdx.x, TR, TC, lower)) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int q = blockIdx.y * 32 + lane;
+  const bool q_ok = q < naux;
+  __shared__ double rho_sh[8][32];
+  double rsum = 0.0;
+  for (int rr = 0; rr < 4; ++rr) {
+    const int R = TR * 32 + warp + 8 * rr;
+    if (R >= nao) break;
+    uint32_t hm = 0;
+    const int c_end = min(32, nao - TC * 32);
+#pragma unroll 8
+    for (int cc = 0; cc < c_end; ++cc) {
+      const int C = TC * 32 + cc;
+      const double x = q_ok ? __ldg(Bp + packed_row(R, C) * naux + q) : 0.0;
+      hm = max(hm, abs_hi_word(x));
+      if (lower && C <= R) {
+        const double d = 0.5 * (__ldg(D + (long long)R * nao + C) + __ldg(D + (long long)C * nao + R));
+        rsum = fma((R == C) ? d : 2.0 * d, x, rsum);
+      }
+    }
+    if (q_ok) atomicMax(&emax[(long long)R * naux + q], hm);
+  }
+  if (lower) {
+    rho_sh[warp][lane] = rsum;
+    __syncthreads();
+    if (warp == 0 && q_ok) {
+      double t = 0.0;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) t += rho_sh[w][lane];
+      atomicAdd(&rho[q], t);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) jk_j_gemv_kernel(const double* __restrict__ Bp, long long npair, int naux,
+                                                        const double* __restrict__ rho, double* __restrict__ Jp) {
+  const int lane = threadIdx.x & 31;
+  const long long p = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (p >= npair) return;
+  const double* b = Bp + p * naux;
+  double acc = 0.0;
+  for (int q = lane; q < naux; q += 32) acc = fma(__ldg(b + q), __ldg(rho + q), acc);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (lane == 0) Jp[p] = acc;
+}
+
+template <int S>
+__global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __restrict__ Bp, int nao, int naux,
+                                                              int q0, int q1, const uint32_t* __restrict__ emax,
+                                                              int32_t* __restrict__ e5, int8_t* __restrict__ planes,
+                                                              long long pitch, long long plane_stride,
+                                                              int* __restrict__ status) {
+  int TR, TC;
+  bool lower;
+  if (!tile_of_block(blockIdx.x, TR, TC, lower)) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int q = q0 + blockIdx.y * 32 + lane;
+  if (q >= q1) return;
+  for (int rr = 0; rr < 4; ++rr) {
+    const int R = TR * 32 + warp + 8 * rr;
+    if (R >= nao) break;
+    const uint32_t hm = emax[(long long)R * naux + q];
+    const int e = scale_index_from_hi(hm);
+    const long long orow = (long long)(q - q0) * nao + R;
+    if (TC == 0) {
+      e5[orow] = e;
+      const int stt = status_from_hi(hm);
+      if (stt) atomicOr(status, stt);
+    }
+    const double scale = pow2_double(63 - e);
+    uint32_t w[S][8];
+#pragma unroll
+    for (int t = 0; t < S; ++t)
+#pragma unroll
+      for (int j = 0; j < 8; ++j) w[t][j] = 0;
+#pragma unroll
+    for (int cc = 0; cc < 32; ++cc) {
+      const int C = TC * 32 + cc;
+      const double x = (C < nao) ? __ldg(Bp + packed_row(R, C) * naux + q) : 0.0;
+      const uint64_t dg = balanced_digits(x, scale);
+#pragma unroll
+      for (int t = 0; t < S; ++t) w[t][cc >> 2] |= digit_byte(dg, t) << (8 * (cc & 3));
+    }
+#pragma unroll
+    for (int t = 0; t < S; ++t) {
+      uint4* dst = reinterpret_cast<uint4*>(planes + t * plane_stride + orow * pitch + TC * 32);
+      dst[0] = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+      dst[1] = make_uint4(w[t][4], w[t][5], w[t][6], w[t][7]);
+    }
+  }
+}
+
+// e6[g][i] from the running maxima GEMM(5)'s epilogue left in xmax[g][i].
+__global__ void jk_x_scale_kernel(const uint32_t* __restrict__ xmax, long long n, int32_t* __restrict__ e6,
+                                  int* __restrict__ status) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const uint32_t m = xmax[t];
+  e6[t] = scale_index_from_hi(m);
+  const int stt = status_from_hi(m);
+  if (stt) atomicOr(status, stt);
+}
+
+// X[i][col] -> planes6[t][i][col]; a thread converts 16 consecutive columns (never straddling a
+// q, hence never a group, because a_pad is a multiple of 16).
+template <int S>
+__global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restrict__ X, int nao, long long ncol,
+                                                         long long ldx, int ng, const int* __restrict__ gcol,
+                                                         const int32_t* __restrict__ e6,
+                                                         int8_t* __restrict__ planes, long long pitch,
+                                                         long long plane_stride) {
+  const int i = blockIdx.y;
+  const long long run = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long c0 = run * 16;
+  if (c0 >= pitch) return;
+  uint32_t w[S][4];
+#pragma unroll
+  for (int t = 0; t < S; ++t)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) w[t][j] = 0;
+  if (c0 < ncol) {
+    int lo = 0, hi = ng - 1;  // largest g with gcol[g] <= c0
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (gcol[mid] <= c0) lo = mid; else hi = mid - 1;
+    }
+    const double scale = pow2_double(63 - e6[(long long)lo * nao + i]);
+    const double2* src = reinterpret_cast<const double2*>(X + (long long)i * ldx + c0);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const double2 v = __ldg(src + j);
+      const uint64_t d0 = balanced_digits(v.x, scale), d1 = balanced_digits(v.y, scale);
+#pragma unroll
+      for (int t = 0; t < S; ++t) {
+        w[t][j >> 1] |= digit_byte(d0, t) << (8 * ((2 * j) & 3));
+        w[t][j >> 1] |= digit_byte(d1, t) << (8 * ((2 * j + 1) & 3));
+      }
+    }
+  }
+#pragma unroll
+  for (int t = 0; t < S; ++t)
+    *reinterpret_cast<uint4*>(planes + t * plane_stride + (long long)i * pitch + c0) =
+        make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+}
+
+// K[i][j] (+)= sum_g Kpart[g][i][j] for column tile <= row tile (tile = 128), mirrored to [j][i].
+__global__ void __launch_bounds__(256) jk_k_reduce_kernel(const double* __restrict__ Kpart, int ng, int nao,
+                                                          int accumulate, double* __restrict__ K) {
+  const int i = blockIdx.y;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nao || (j / kTileM) > (i / kTileM)) return;
+  const long long nn = (long long)nao * nao;
+  const long long ij = (long long)i * nao + j;
+  double acc = accumulate ? K[ij] : 0.0;
+  for (int g = 0; g < ng; ++g) acc += Kpart[g * nn + ij];
+  K[ij] = acc;
+  if ((j / kTileM) < (i / kTileM)) K[(long long)j * nao + i] = acc;
+}
+
+__global__ void __launch_bounds__(256) jk_j_unpack_kernel(const double* __restrict__ Jp, int nao,
+                                                          double* __restrict__ J) {
+  const int i = blockIdx.y;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nao) return;
+  J[(long long)i * nao + j] = Jp[packed_row(i, j)];
+}
+
+// ---------------------------------------------------------------------------
+static unsigned tile_blocks(int nao) {
+  const unsigned T = (unsigned)((nao + 31) / 32);
+  return T * (T + 1);  // 2 * T(T+1)/2
+}
+
+cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho, uint32_t* emax,
+                             cudaStream_t st) {
+  dim3 grid(tile_blocks(nao), (unsigned)((naux + 31) / 32));
+  jk_pass_a_kernel<<<grid, 256, 0, st>>>(Bp, nao, naux, D, rho, emax);
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const double* rho, double* Jp,
+                             cudaStream_t st) {
+  jk_j_gemv_kernel<<<(unsigned)((npair + 7) / 8), 256, 0, st>>>(Bp, npair, naux, rho, Jp);
+  count_launch();
+  return cudaGetLastError();
+}
+
+#define DFE_DISPATCH_S(S_, CALL)      \
+  switch (S_) {                       \
+    case 1: { constexpr int SS = 1; CALL; } break; \
+    case 2: { constexpr int SS = 2; CALL; } break; \
+    case 3: { constexpr int SS = 3; CALL; } break; \
+    case 4: { constexpr int SS = 4; CALL; } break; \
+    case 5: { constexpr int SS = 5; CALL; } break; \
+    case 6: { constexpr int SS = 6; CALL; } break; \
+    case 7: { constexpr int SS = 7; CALL; } break; \
+    default: { constexpr int SS = 8; CALL; } break; \
+  }
+
+cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
+                                   int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
+                                   int* status, cudaStream_t st) {
+  dim3 grid(tile_blocks(nao), (unsigned)((q1 - q0 + 31) / 32));
+  DFE_DISPATCH_S(s, (jk_unpack_split_kernel<SS><<<grid, 256, 0, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5,
+                                                                      pitch, plane_stride, status)));
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_jk_split_x(const double* X, int nao, int64_t ncol, int64_t ldx, int s, int ng, const int* gcol,
+                              const uint32_t* xmax, int32_t* e6, int8_t* planes6, int64_t pitch6,
+                              int64_t plane_stride6, int* status, cudaStream_t st) {
+  const long long n = (long long)ng * nao;
+  jk_x_scale_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(xmax, n, e6, status);
+  dim3 grid((unsigned)((pitch6 / 16 + 255) / 256), (unsigned)nao);
+  DFE_DISPATCH_S(s, (jk_split_x_kernel<SS><<<grid, 256, 0, st>>>(X, nao, ncol, ldx, ng, gcol, e6, planes6, pitch6,
+                                                                 plane_stride6)));
+  count_launch(2);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_jk_k_reduce(const double* Kpart, int ng, int nao, int accumulate, double* K, cudaStream_t st) {
+  dim3 grid((unsigned)((nao + 255) / 256), (unsigned)nao);
+  jk_k_reduce_kernel<<<grid, 256, 0, st>>>(Kpart, ng, nao, accumulate, K);
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_jk_j_unpack(const double* Jp, int nao, double* J, cudaStream_t st) {
+  dim3 grid((unsigned)((nao + 255) / 256), (unsigned)nao);
+  jk_j_unpack_kernel<<<grid, 256, 0, st>>>(Jp, nao, J);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace dfe
