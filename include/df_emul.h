@@ -80,6 +80,10 @@ int64_t df_emul_gemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int s);
  * batch several 512-blocks per launch. */
 int64_t df_jk_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, int s);
 
+/* Bytes needed to batch `nblocks` 512-q blocks per launch (nblocks >= ceil(naux/512)
+ * = the whole auxiliary range in one super-block). */
+int64_t df_jk_workspace_bytes_blocks(int64_t nao, int64_t naux, int64_t nocc, int s, int64_t nblocks);
+
 /* Register a device buffer (256-byte aligned) as THE workspace.  The library
  * never frees it.  Passing NULL/0 unregisters it. */
 int df_set_workspace(void* ptr, int64_t bytes);
@@ -152,6 +156,17 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
 
 /* Number of GPU kernels this library has launched in this process. */
 int64_t df_launch_count(void);
+
+/* Per-kernel-class device timing for the roofline report (bench.py).  While
+ * enabled, every entry point brackets each kernel class it launches with a pair
+ * of CUDA events on the caller's stream.  df_profile_read() SYNCHRONISES on the
+ * recorded events, returns the summed milliseconds and the number of brackets
+ * per class since the last read in ms_by_class[df_profile_num_classes()] /
+ * count_by_class[...] (host arrays), and clears the records. */
+int df_profile_enable(int on);
+int df_profile_num_classes(void);
+const char* df_profile_class_name(int cls);
+int df_profile_read(float* ms_by_class, int* count_by_class);
 
 /* Back-to-back tcgen05.mma.kind::i8 issue-rate probe (operands resident in
  * shared memory, no loads): runs `iters` MMAs of shape 128 x n_mma x 32 per CTA

@@ -44,6 +44,7 @@ _SIG = {
     "df_plane_pitch": (_i64, [_i64]),
     "df_emul_gemm_workspace_bytes": (_i64, [_i64, _i64, _i64, _i32]),
     "df_jk_workspace_bytes": (_i64, [_i64, _i64, _i64, _i32]),
+    "df_jk_workspace_bytes_blocks": (_i64, [_i64, _i64, _i64, _i32, _i64]),
     "df_set_workspace": (_i32, [_vp, _i64]),
     "df_emul_gemm": (_i32, [_vp, _vp, _vp, _i64, _i64, _i64, _f64, _vp]),
     "df_emul_gemm_slices": (_i32, [_vp, _vp, _vp, _i64, _i64, _i64, _i32, _vp]),
@@ -56,6 +57,10 @@ _SIG = {
     "df_debug_jk_build": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp, _vp,
                                  C.POINTER(C.c_int), _vp]),
     "df_launch_count": (_i64, []),
+    "df_profile_enable": (_i32, [_i32]),
+    "df_profile_num_classes": (_i32, []),
+    "df_profile_class_name": (C.c_char_p, [_i32]),
+    "df_profile_read": (_i32, [C.POINTER(C.c_float), C.POINTER(C.c_int)]),
     "df_debug_mma_peak": (_i32, [_i32, _i32, _i32, C.POINTER(C.c_float), _vp]),
 }
 EXPORTS = tuple(_SIG)
@@ -116,6 +121,10 @@ def df_emul_gemm_workspace_bytes(m: int, n: int, k: int, s: int) -> int:
 
 def df_jk_workspace_bytes(nao: int, naux: int, nocc: int, s: int) -> int:
     return _check(lib.df_jk_workspace_bytes(nao, naux, nocc, s), "df_jk_workspace_bytes")
+
+
+def df_jk_workspace_bytes_blocks(nao: int, naux: int, nocc: int, s: int, nblocks: int) -> int:
+    return _check(lib.df_jk_workspace_bytes_blocks(nao, naux, nocc, s, nblocks), "df_jk_workspace_bytes_blocks")
 
 
 def df_set_workspace(buf) -> None:
@@ -215,6 +224,19 @@ def df_debug_jk_build(B_packed, nao, naux, C_occ, nocc, D, s, J, K, X_out=None, 
 
 def df_launch_count() -> int:
     return int(lib.df_launch_count())
+
+
+def df_profile_enable(on: bool) -> None:
+    _check(lib.df_profile_enable(1 if on else 0), "df_profile_enable")
+
+
+def df_profile_read() -> dict:
+    """{class name: (milliseconds, brackets)} since the last read; synchronises."""
+    n = int(lib.df_profile_num_classes())
+    ms = (C.c_float * n)()
+    cnt = (C.c_int * n)()
+    _check(lib.df_profile_read(ms, cnt), "df_profile_read")
+    return {lib.df_profile_class_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(n)}
 
 
 def df_debug_mma_peak(n_mma: int, iters: int, grid: int, stream=None) -> float:

@@ -6,6 +6,7 @@
 #include <stdint.h>
 
 #include <atomic>
+#include <vector>
 
 #include "../../include/df_emul.h"
 #include "internal.h"
@@ -19,6 +20,47 @@ static void* g_ws = nullptr;
 static int64_t g_ws_bytes = 0;
 static int g_mode = DF_MODE_GUARDED;
 static int g_device_ok = -1;
+
+// ---- optional per-kernel-class CUDA-event timing (df_profile_*; bench.py's roofline) ----
+enum ProfClass { kPSplit = 0, kPPassA, kPJGemv, kPUnpack, kPGemm5, kPSplitX, kPGemm6, kPReduce, kPGemm, kPNum };
+static const char* const kProfNames[kPNum] = {"split",   "jk_pass_a", "jk_j_gemv", "jk_unpack_split", "gemm5_i8",
+                                              "jk_split_x", "gemm6_i8",  "jk_k_reduce", "emul_gemm_i8"};
+struct ProfRec {
+  int cls;
+  cudaEvent_t e0, e1;
+};
+static bool g_prof_on = false;
+static std::vector<ProfRec> g_prof_recs;    // records of the current profiling window
+static std::vector<cudaEvent_t> g_prof_pool;  // recycled events
+static cudaEvent_t prof_event() {
+  cudaEvent_t e;
+  if (!g_prof_pool.empty()) {
+    e = g_prof_pool.back();
+    g_prof_pool.pop_back();
+  } else {
+    cudaEventCreate(&e);
+  }
+  return e;
+}
+struct ProfScope {
+  cudaStream_t st;
+  bool on;
+  ProfRec r;
+  ProfScope(int cls, cudaStream_t s) : st(s), on(g_prof_on) {
+    if (on) {
+      r.cls = cls;
+      r.e0 = prof_event();
+      r.e1 = prof_event();
+      cudaEventRecord(r.e0, st);
+    }
+  }
+  ~ProfScope() {
+    if (on) {
+      cudaEventRecord(r.e1, st);
+      g_prof_recs.push_back(r);
+    }
+  }
+};
 
 static int device_ok() {
   if (g_device_ok < 0) {
@@ -101,10 +143,13 @@ static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m
   GemmWs w = carve_gemm(g_ws, m, n, k, s);
   if (w.bytes > g_ws_bytes) return DF_ERR_WORKSPACE;
 
-  if (launch_split_rows(A, m, k, k, s, w.eA, w.pa, w.pitch, m * w.pitch, w.status, st) != cudaSuccess)
-    return DF_ERR_CUDA;
-  if (launch_split_cols(B, k, n, s, w.cmax, w.eB, w.pb, w.pitch, n * w.pitch, w.status, st) != cudaSuccess)
-    return DF_ERR_CUDA;
+  {
+    ProfScope ps(kPSplit, st);
+    if (launch_split_rows(A, m, k, k, s, w.eA, w.pa, w.pitch, m * w.pitch, w.status, st) != cudaSuccess)
+      return DF_ERR_CUDA;
+    if (launch_split_cols(B, k, n, s, w.cmax, w.eB, w.pb, w.pitch, n * w.pitch, w.status, st) != cudaSuccess)
+      return DF_ERR_CUDA;
+  }
 
   GemmProblem g = {};
   g.A = w.pa;
@@ -125,7 +170,10 @@ static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m
   g.mode = kEpiC;
   g.C = C;
   g.ldc = n;
-  if (launch_gemm_i8(g, st) != cudaSuccess) return DF_ERR_CUDA;
+  {
+    ProfScope ps(kPGemm, st);
+    if (launch_gemm_i8(g, st) != cudaSuccess) return DF_ERR_CUDA;
+  }
   return DF_OK;
 }
 
@@ -200,7 +248,7 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
                    int s, double* J, double* K, double* X_out, int32_t* e6_out, int* ngroups_out,
                    cudaStream_t st) {
   if (!Bp || !Cocc || !D || !J || !K) return DF_ERR_NULL;
-  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nao > 32768 || naux > (1 << 20)) return DF_ERR_DIM;
+  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nao > 8160 || naux > (1 << 20)) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
   if (!device_ok()) return DF_ERR_DEVICE;
   if (!g_ws) return DF_ERR_WORKSPACE;
@@ -228,15 +276,24 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
   // ---- J: rho (Eq. 3) fused with GEMM(5)'s row maxima, then J (Eq. 4) ----
   DFE_CK(cudaMemsetAsync(w.rho, 0, sizeof(double) * naux, st));
   DFE_CK(cudaMemsetAsync(w.emax5, 0, sizeof(uint32_t) * nao * naux, st));
-  DFE_CK(launch_jk_pass_a(Bp, (int)nao, (int)naux, D, w.rho, w.emax5, st));
-  DFE_CK(launch_jk_j_gemv(Bp, npair, (int)naux, w.rho, w.Jp, st));
-  DFE_CK(launch_jk_j_unpack(w.Jp, (int)nao, J, st));
+  {
+    ProfScope ps(kPPassA, st);
+    DFE_CK(launch_jk_pass_a(Bp, (int)nao, (int)naux, D, w.rho, w.emax5, st));
+  }
+  {
+    ProfScope ps(kPJGemv, st);
+    DFE_CK(launch_jk_j_gemv(Bp, npair, (int)naux, w.rho, w.Jp, st));
+    DFE_CK(launch_jk_j_unpack(w.Jp, (int)nao, J, st));
+  }
 
   // ---- right operand of GEMM(5): C_occ columns -> K-major planes, a_pad rows (padding rows 0) ----
   DFE_CK(cudaMemsetAsync(w.eC, 0, sizeof(int32_t) * w.a_pad, st));
   DFE_CK(cudaMemsetAsync(w.pc, 0, (size_t)s * w.a_pad * w.pitchj, st));
-  DFE_CK(launch_split_cols(Cocc, nao, nocc, s, w.cmaxC, w.eC, w.pc, w.pitchj, (int64_t)w.a_pad * w.pitchj,
-                           w.status, st));
+  {
+    ProfScope ps(kPSplit, st);
+    DFE_CK(launch_split_cols(Cocc, nao, nocc, s, w.cmaxC, w.eC, w.pc, w.pitchj, (int64_t)w.a_pad * w.pitchj,
+                             w.status, st));
+  }
 
   int gtotal = 0;
   for (int64_t qs0 = 0; qs0 < naux; qs0 += QS) {
@@ -253,8 +310,11 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     DFE_CK(cudaMemsetAsync(w.xmax, 0, sizeof(uint32_t) * ng * nao, st));
 
     // H2: unpack + split packed B -> planes5 rows (q, i), contraction j
-    DFE_CK(launch_jk_unpack_split(Bp, (int)nao, (int)naux, (int)qs0, (int)qs1, w.emax5, s, w.e5, w.p5, w.pitchj,
-                                  (int64_t)nq * nao * w.pitchj, w.status, st));
+    {
+      ProfScope ps(kPUnpack, st);
+      DFE_CK(launch_jk_unpack_split(Bp, (int)nao, (int)naux, (int)qs0, (int)qs1, w.emax5, s, w.e5, w.p5,
+                                    w.pitchj, (int64_t)nq * nao * w.pitchj, w.status, st));
+    }
     // GEMM(5): X[i][q][a] = sum_j B^q_ij C_ja   (Eq. 5 / Eq. 12)
     GemmProblem g5 = {};
     g5.A = w.p5;
@@ -276,14 +336,20 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     g5.ldx = ncol;
     g5.qgroup = w.qgroup;
     g5.xmax = w.xmax;
-    DFE_CK(launch_gemm_i8(g5, st));
+    {
+      ProfScope ps(kPGemm5, st);
+      DFE_CK(launch_gemm_i8(g5, st));
+    }
     if (X_out)
       DFE_CK(cudaMemcpy2DAsync(X_out + qs0 * w.a_pad, sizeof(double) * naux * w.a_pad, w.X, sizeof(double) * ncol,
                                sizeof(double) * ncol, nao, cudaMemcpyDeviceToDevice, st));
 
     // X -> planes6 with one scale per (i, group)
-    DFE_CK(launch_jk_split_x(w.X, (int)nao, ncol, ncol, s, ng, w.gcol, w.xmax, w.e6, w.p6, pitch6,
-                             (int64_t)nao * pitch6, w.status, st));
+    {
+      ProfScope ps(kPSplitX, st);
+      DFE_CK(launch_jk_split_x(w.X, (int)nao, ncol, ncol, s, ng, w.gcol, w.xmax, w.e6, w.p6, pitch6,
+                               (int64_t)nao * pitch6, w.status, st));
+    }
     if (e6_out)
       DFE_CK(cudaMemcpyAsync(e6_out + (int64_t)gtotal * nao, w.e6, sizeof(int32_t) * ng * nao,
                              cudaMemcpyDeviceToDevice, st));
@@ -308,9 +374,15 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     g6.C = w.Kpart;
     g6.ldc = nao;
     g6.c_stride = nao * nao;
-    DFE_CK(launch_gemm_i8(g6, st));
+    {
+      ProfScope ps(kPGemm6, st);
+      DFE_CK(launch_gemm_i8(g6, st));
+    }
     // H7: K += sum_g K_g in increasing-q order, mirrored to the upper triangle
-    DFE_CK(launch_jk_k_reduce(w.Kpart, ng, (int)nao, qs0 > 0 ? 1 : 0, K, st));
+    {
+      ProfScope ps(kPReduce, st);
+      DFE_CK(launch_jk_k_reduce(w.Kpart, ng, (int)nao, qs0 > 0 ? 1 : 0, K, st));
+    }
     gtotal += ng;
   }
   if (ngroups_out) *ngroups_out = gtotal;
@@ -354,6 +426,14 @@ int64_t df_jk_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, int s) {
   if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
   const int64_t qs = naux < kQBlock ? naux : kQBlock;
+  return carve_jk(nullptr, nao, naux, nocc, s, qs).bytes;
+}
+
+int64_t df_jk_workspace_bytes_blocks(int64_t nao, int64_t naux, int64_t nocc, int s, int64_t nblocks) {
+  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nblocks < 1) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  int64_t qs = nblocks * kQBlock;
+  if (qs > naux) qs = naux;
   return carve_jk(nullptr, nao, naux, nocc, s, qs).bytes;
 }
 
@@ -470,6 +550,35 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t 
 }
 
 int64_t df_launch_count(void) { return (int64_t)g_launches.load(); }
+
+int df_profile_enable(int on) {
+  g_prof_on = on != 0;
+  return DF_OK;
+}
+
+int df_profile_num_classes(void) { return kPNum; }
+
+const char* df_profile_class_name(int cls) { return (cls < 0 || cls >= kPNum) ? "" : kProfNames[cls]; }
+
+int df_profile_read(float* ms_by_class, int* count_by_class) {
+  if (!ms_by_class || !count_by_class) return DF_ERR_NULL;
+  for (int i = 0; i < kPNum; ++i) {
+    ms_by_class[i] = 0.f;
+    count_by_class[i] = 0;
+  }
+  int rc = DF_OK;
+  for (ProfRec& r : g_prof_recs) {
+    float ms = 0.f;
+    if (cudaEventSynchronize(r.e1) != cudaSuccess || cudaEventElapsedTime(&ms, r.e0, r.e1) != cudaSuccess)
+      rc = DF_ERR_CUDA;
+    ms_by_class[r.cls] += ms;
+    count_by_class[r.cls] += 1;
+    g_prof_pool.push_back(r.e0);
+    g_prof_pool.push_back(r.e1);
+  }
+  g_prof_recs.clear();
+  return rc;
+}
 
 int df_debug_mma_peak(int n_mma, int iters, int grid, float* ms, void* stream) {
   if (!ms) return DF_ERR_NULL;

@@ -81,6 +81,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   __shared__ __align__(8) uint64_t tmem_full_bar;
   __shared__ __align__(8) uint64_t tmem_empty_bar;
   __shared__ uint32_t tmem_slot;
+  __shared__ uint4 pair_tab[kMaxSlices * (kMaxSlices + 1) / 2];
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -150,8 +151,15 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     }
   } else if (warp == 1) {
     // ================= MMA issuer =================
+    // One thread issues every MMA, so the per-MMA instruction count must stay far below the
+    // MMA's own duration (64 cycles at N = 128): the (t, u, w) loop nest is flattened once per
+    // pass into a table {A plane offset, B plane offset, accumulator column, accumulate flag},
+    // and the inner loop only adds the K offset to the descriptors' address fields.
     if (lane == 0) {
       const uint32_t idesc = make_idesc_i8(kTileM, p.n_tile);
+      const uint64_t desc_proto = make_smem_desc(0, BK);
+      const uint32_t desc_hi = (uint32_t)(desc_proto >> 32);
+      const uint32_t desc_lo0 = (uint32_t)desc_proto;  // LBO field, address 0
       uint32_t it = 0, iter = 0;
       for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
         const int kc0 = zk0 + ch * p.kflush;
@@ -160,6 +168,14 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         for (int ps = 0; ps < npass; ++ps, ++iter) {
           int w_hi, w_lo;
           pass_weights(s, W, ps, w_hi, w_lo);
+          int np = 0;
+          for (int w = w_hi; w >= w_lo; --w) {
+            const int t_lo = max(1, w - s), t_hi = min(s, w - 1);
+            for (int t = t_lo; t <= t_hi; ++t, ++np)
+              pair_tab[np] = make_uint4(((uint32_t)(t - 1) * a_plane_bytes) >> 4,
+                                        (b_off + (uint32_t)(w - t - 1) * b_plane_bytes) >> 4,
+                                        tmem_base + (uint32_t)((w_hi - w) * p.acc_stride), t > t_lo ? 1u : 0u);
+          }
           if (iter > 0) {
             mbar_wait(&tmem_empty_bar, (iter - 1) & 1u);
             tc_fence_after();
@@ -170,19 +186,18 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             mbar_wait(&full_bar[stage], ph);
             tc_fence_after();
             const uint32_t sa = smem_u32(smem + (size_t)stage * p.stage_stride);
+            const uint32_t lo_base = desc_lo0 | ((sa & 0x3FFFFu) >> 4);
             const int kpos = kc0 + kb * BK;
             const int nkk = (min(BK, kc1 - kpos) + 31) / 32;
             for (int kk = 0; kk < nkk; ++kk) {
-              for (int w = w_hi; w >= w_lo; --w) {
-                const int t_lo = max(1, w - s), t_hi = min(s, w - 1);
-                const uint32_t d_tmem = tmem_base + (uint32_t)((w_hi - w) * p.acc_stride);
-                for (int t = t_lo; t <= t_hi; ++t) {
-                  const int u = w - t;
-                  const uint64_t adesc = make_smem_desc(sa + (t - 1) * a_plane_bytes + kk * 32, BK);
-                  const uint64_t bdesc = make_smem_desc(sa + b_off + (u - 1) * b_plane_bytes + kk * 32, BK);
-                  const uint32_t acc = (kb > 0 || kk > 0 || t > t_lo) ? 1u : 0u;
-                  mma_i8_ss(d_tmem, adesc, bdesc, idesc, acc);
-                }
+              const uint32_t lo = lo_base + 2u * kk;  // +32 bytes per K step, in 16-byte units
+              const uint32_t later = (kb | kk) ? 1u : 0u;
+#pragma unroll 4
+              for (int i = 0; i < np; ++i) {
+                const uint4 e = pair_tab[i];
+                const uint64_t adesc = ((uint64_t)desc_hi << 32) | (lo + e.x);
+                const uint64_t bdesc = ((uint64_t)desc_hi << 32) | (lo + e.y);
+                mma_i8_ss(e.z, adesc, bdesc, idesc, later | e.w);
               }
             }
             mma_commit(&empty_bar[stage]);  // frees the smem stage once these MMAs have read it

@@ -47,9 +47,9 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
                                                         uint32_t* __restrict__ emax) {
   int TR, TC;
   bool lower;
-  if (!tile_of_block(blockIdx.x, TR, TC, lower)) return;
+  if (!tile_of_block(blockIdx.y, TR, TC, lower)) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = blockIdx.y * 32 + lane;
+  const int q = blockIdx.x * 32 + lane;  // q chunk fastest: concurrent blocks read adjacent runs of a row
   const bool q_ok = q < naux;
   __shared__ double rho_sh[8][32];
   double rsum = 0.0;
@@ -103,9 +103,9 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
                                                               int* __restrict__ status) {
   int TR, TC;
   bool lower;
-  if (!tile_of_block(blockIdx.x, TR, TC, lower)) return;
+  if (!tile_of_block(blockIdx.y, TR, TC, lower)) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = q0 + blockIdx.y * 32 + lane;
+  const int q = q0 + blockIdx.x * 32 + lane;
   if (q >= q1) return;
   for (int rr = 0; rr < 4; ++rr) {
     const int R = TR * 32 + warp + 8 * rr;
@@ -224,7 +224,7 @@ static unsigned tile_blocks(int nao) {
 
 cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho, uint32_t* emax,
                              cudaStream_t st) {
-  dim3 grid(tile_blocks(nao), (unsigned)((naux + 31) / 32));
+  dim3 grid((unsigned)((naux + 31) / 32), tile_blocks(nao));
   jk_pass_a_kernel<<<grid, 256, 0, st>>>(Bp, nao, naux, D, rho, emax);
   count_launch();
   return cudaGetLastError();
@@ -252,7 +252,7 @@ cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const do
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
                                    int* status, cudaStream_t st) {
-  dim3 grid(tile_blocks(nao), (unsigned)((q1 - q0 + 31) / 32));
+  dim3 grid((unsigned)((q1 - q0 + 31) / 32), tile_blocks(nao));
   DFE_DISPATCH_S(s, (jk_unpack_split_kernel<SS><<<grid, 256, 0, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5,
                                                                       pitch, plane_stride, status)));
   count_launch();

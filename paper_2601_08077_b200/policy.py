@@ -1,0 +1,52 @@
+"""Caller side of the tolerance policy (row H0 of SURVEY.md 8(a)): the adaptive schedule of
+PAPER.md:132-151.  After SCF iteration i the caller computes dE_rel,i (Eq. 11),
+looks it up in Table 1 and passes the resulting emulation accuracy as `tol`
+to df_jk_build for iteration i+1; precision never goes back down and iteration 0 starts at
+m_emu = 23.  The library then maps tol -> slices (df_slices_for_tol).
+
+Host-only, no arithmetic of the method itself; the table is typed from the paper.
+"""
+from __future__ import annotations
+
+# (lower bound of dE_rel, emulation level, mantissa bits m_emu)
+TABLE1 = ((2e-6, 4, 23), (5e-9, 3, 31), (2e-11, 2, 39), (7e-14, 1, 47))
+M_EMU_OF_LEVEL = {4: 23, 3: 31, 2: 39, 1: 47, 0: 52}  # level 0 = native FP64 (2^-52 = 2.2e-16)
+START_LEVEL = 4
+
+
+def level_for(dE_rel: float) -> int:
+    """Emulation level for the NEXT iteration given this iteration's relative energy change."""
+    for lo, level, _ in TABLE1:
+        if dE_rel >= lo:
+            return level
+    return 0
+
+
+def tol_of_level(level: int) -> float:
+    """Table 1's "Emu. Relative Accuracy" column: 2^-m_emu."""
+    return 2.0 ** (-M_EMU_OF_LEVEL[level])
+
+
+class AdaptiveTolerance:
+    """tol for each SCF iteration; feed it dE_rel after every iteration."""
+
+    def __init__(self):
+        self.level = START_LEVEL
+
+    @property
+    def tol(self) -> float:
+        return tol_of_level(self.level)
+
+    def update(self, dE_rel: float) -> float:
+        self.level = min(self.level, level_for(abs(dE_rel)))  # never revert
+        return self.tol
+
+
+def schedule(dE_rels):
+    """[(level, tol)] for iterations 0..len(dE_rels): iteration i+1 uses dE_rel of iteration i."""
+    a = AdaptiveTolerance()
+    out = [(a.level, a.tol)]
+    for d in dE_rels:
+        a.update(d)
+        out.append((a.level, a.tol))
+    return out

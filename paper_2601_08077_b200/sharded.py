@@ -1,0 +1,45 @@
+"""q-sharded multi-GPU J/K build: one process per GPU, each rank holds
+the columns B[:, q0:q1] of its own auxiliary-index range.  rho_q is local to its shard
+(PAPER.md:45), J and K are sums over q, so the only exchange step is one
+all-reduce(sum) of J and of K per build -- over NCCL/NVLink on GPUs, gloo in the CPU tests.
+
+Shards are multiples of the 512-q block of the K path (R5), so the q-groups -- and
+with them every INT8 digit -- are the same as in the single-GPU build.
+"""
+from __future__ import annotations
+
+QBLOCK = 512
+
+
+def shard_range(naux: int, rank: int, world: int, qblock: int = QBLOCK):
+    """[q0, q1) of `rank`: 512-q blocks dealt out as evenly as possible, in order."""
+    if not (0 <= rank < world):
+        raise ValueError("rank out of range")
+    nblk = (naux + qblock - 1) // qblock
+    base, extra = divmod(nblk, world)
+    b0 = rank * base + min(rank, extra)
+    b1 = b0 + base + (1 if rank < extra else 0)
+    return min(naux, b0 * qblock), min(naux, b1 * qblock)
+
+
+def allreduce_jk(J, K, group=None):
+    """The exchange step: J and K partial sums over this rank's q range -> full J, K (in place)."""
+    import torch.distributed as dist
+
+    if dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(J, op=dist.ReduceOp.SUM, group=group)
+        dist.all_reduce(K, op=dist.ReduceOp.SUM, group=group)
+    return J, K
+
+
+def df_jk_build_sharded(B_shard, nao, naux_shard, C_occ, nocc, D, tol, J, K, group=None, stream=None):
+    """This rank's df_jk_build over its shard of q (B_shard = B_packed[:, q0:q1], contiguous),
+    then the all-reduce.  With an empty shard the rank contributes zeros."""
+    from . import binding
+
+    if naux_shard > 0:
+        binding.df_jk_build(B_shard, nao, naux_shard, C_occ, nocc, D, tol, J, K, stream)
+    else:
+        J.zero_()
+        K.zero_()
+    return allreduce_jk(J, K, group)

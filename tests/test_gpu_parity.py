@@ -1,0 +1,276 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by
+element on the same seeded inputs.  Integer work (scale indices, digits, INT32 weight sums) is
+bit-exact; the emulated FP64 GEMM follows the oracle's summation order, so it is compared
+bit-exactly too (R6) and, separately, within the requested tol against plain FP64."""
+import numpy as np
+import pytest
+import torch
+
+from df_inputs import generators as G
+from oracle import df_oracle as O
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+TOLS = (1e-4, 1e-6, 1e-8, 1e-10)  # BASELINE.json north_star
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).to(DEV)
+
+
+def edge_matrix(rows, cols, seed):
+    """Random wide-range rows plus the scale-index edge cases of DESIGN.md R2."""
+    rng = np.random.default_rng(seed)
+    X = rng.standard_normal((rows, cols)) * np.exp2(rng.integers(-25, 25, size=(rows, 1)).astype(float))
+    X *= np.exp2(rng.uniform(-20, 0, size=(rows, cols)))
+    X[0] = 0.0                                   # zero row
+    X[1] = 0.0; X[1, cols // 2] = -1.0           # a single power of two
+    X[2] *= 1e-3; X[2, 0] = 127.0 / 128.0        # exactly at the bump boundary f = 127/128
+    X[3] *= 1e-3; X[3, 1] = np.nextafter(127.0 / 128.0, 0.0)  # just below it
+    X[4] *= 1e-3; X[4, 2] = np.nextafter(1.0, 0.0)            # just below a power of two
+    X[5] = 2.0 ** -1005                          # below the tiny-row threshold -> zero row
+    X[6, :] = np.where(rng.integers(0, 2, cols) > 0, 1.0, -1.0) * 2.0 ** 17  # +-max everywhere
+    X[7] = 0.0; X[7, -1] = 3.0e-300              # valid scale, flagged out of range
+    return X
+
+
+@pytest.mark.parametrize("rows,cols", [(37, 1000), (130, 48), (9, 17), (64, 4099)])
+@pytest.mark.parametrize("s", [1, 3, 8])
+def test_split_rows_bit_exact(dfe, gpu_ws, rows, cols, s):
+    X = edge_matrix(max(rows, 8), cols, seed=rows + cols)
+    rows = X.shape[0]
+    e_ref, D_ref = O.split_operand(X, s)
+    pitch = dfe.df_plane_pitch(cols)
+    e = torch.empty(rows, dtype=torch.int32, device=DEV)
+    pl = torch.full((s, rows, pitch), 99, dtype=torch.int8, device=DEV)
+    dfe.df_debug_split_rows(dev(X), rows, cols, s, e, pl)
+    torch.cuda.synchronize()
+    assert np.array_equal(e.cpu().numpy(), e_ref)
+    got = pl.cpu().numpy()
+    ok_rows = np.arange(rows) != 7  # row 7 is out of range: flagged, digits unspecified (R9)
+    assert np.array_equal(got[:, ok_rows, :cols], D_ref[:, ok_rows])
+    assert not got[:, :, cols:].any()  # padding is zero
+    assert dfe.df_last_status() == dfe.DF_STATUS_RANGE  # row 7 only
+    assert O.operand_status(X) == 2
+
+
+@pytest.mark.parametrize("k,n", [(1000, 37), (48, 130), (33, 9), (300, 1000)])
+@pytest.mark.parametrize("s", [2, 5, 8])
+def test_split_cols_bit_exact(dfe, gpu_ws, k, n, s):
+    Xt = edge_matrix(max(n, 8), k, seed=k * 3 + n)  # rows = columns of the k x n operand
+    n = Xt.shape[0]
+    X = np.ascontiguousarray(Xt.T)
+    e_ref, D_ref = O.split_operand(Xt, s)
+    pitch = dfe.df_plane_pitch(k)
+    e = torch.empty(n, dtype=torch.int32, device=DEV)
+    pl = torch.full((s, n, pitch), 99, dtype=torch.int8, device=DEV)
+    dfe.df_debug_split_cols(dev(X), k, n, s, e, pl)
+    torch.cuda.synchronize()
+    assert np.array_equal(e.cpu().numpy(), e_ref)
+    got = pl.cpu().numpy()
+    ok_cols = np.arange(n) != 7  # column 7 is out of range: flagged, digits unspecified (R9)
+    assert np.array_equal(got[:, ok_cols, :k], D_ref[:, ok_cols])
+    assert not got[:, :, k:].any()
+    assert dfe.df_last_status() == dfe.DF_STATUS_RANGE
+
+
+def test_status_word_flags_nonfinite(dfe, gpu_ws):
+    X = np.ones((4, 64)); X[2, 5] = np.inf
+    e = torch.empty(4, dtype=torch.int32, device=DEV)
+    pl = torch.empty((2, 4, 64), dtype=torch.int8, device=DEV)
+    dfe.df_last_status()
+    dfe.df_debug_split_rows(dev(X), 4, 64, 2, e, pl)
+    assert dfe.df_last_status() & dfe.DF_STATUS_NONFINITE
+    assert dfe.df_last_status() == 0  # cleared by the read
+    assert O.operand_status(X) & 1
+
+
+def random_digits(s, rows, k, seed):
+    rng = np.random.default_rng(seed)
+    pitch = (k + 31) // 32 * 32
+    D = np.full((s, rows, pitch), 77, dtype=np.int8)  # garbage past k must never be read
+    D[:, :, :k] = rng.integers(-128, 128, size=(s, rows, k))
+    D[:, 0, :k] = -128  # extreme rows: the INT32 guard's worst case
+    D[:, -1, :k] = 127
+    return D
+
+
+@pytest.mark.parametrize("bk", [32, 64, 128])
+@pytest.mark.parametrize("m,n,k,s", [
+    (128, 128, 128, 1),     # one tile, one slice pair: P^(1,1)
+    (300, 200, 1000, 4),    # several tiles, ragged tails in m, n, k
+    (130, 160, 1200, 3),    # GEMM(5)-like: n_tile = 160 -> 3 weights per pass, 1 pass
+    (257, 48, 777, 5),      # narrow N, all 5 weights in TMEM
+    (129, 250, 96, 8),      # two N tiles, two passes of 4 weights
+])
+def test_weight_sums_int32_bit_exact(dfe, gpu_ws, bk, m, n, k, s):
+    DA, DB = random_digits(s, m, k, 11), random_digits(s, n, k, 12)
+    P = torch.full((s, m, n), -12345, dtype=torch.int32, device=DEV)
+    dfe.df_debug_weight_sums(dev(DA), dev(DB), m, n, k, s, 0, bk, P)
+    torch.cuda.synchronize()
+    ref = O.weight_sums(DA[:, :, :k], DB[:, :, :k], s)
+    got = P.cpu().numpy()
+    for w in range(2, s + 2):
+        assert np.array_equal(got[w - 2], ref[w]), f"w={w}"
+
+
+@pytest.mark.parametrize("s,k", [(8, 16352 + 2000), (3, 43680 + 64)])
+def test_weight_sums_flush_chunks(dfe, gpu_ws, s, k):
+    """k > kflush(s): every chunk's INT32 sums are exact and the worst case does not overflow."""
+    m, n = 128, 64
+    DA, DB = random_digits(s, m, k, 21), random_digits(s, n, k, 22)
+    kf = dfe.df_kflush(s)
+    P = torch.empty((s, m, n), dtype=torch.int32, device=DEV)
+    for ch in range((k + kf - 1) // kf):
+        dfe.df_debug_weight_sums(dev(DA), dev(DB), m, n, k, s, ch, 0, P)
+        torch.cuda.synchronize()
+        ref = O.weight_sums(DA[:, :, :k], DB[:, :, :k], s, ch * kf, min(k, (ch + 1) * kf))
+        got = P.cpu().numpy()
+        for w in range(2, s + 2):
+            assert np.abs(ref[w]).max() < 2 ** 31
+            assert np.array_equal(got[w - 2], ref[w]), f"chunk {ch} w={w}"
+
+
+@pytest.mark.parametrize("m,n,k", [(256, 256, 256), (300, 200, 1000), (128, 48, 4096), (1, 1, 1), (5, 700, 33)])
+def test_emul_gemm_matches_oracle_emulation_bitwise(dfe, gpu_ws, m, n, k):
+    A, B = G.make_gemm_inputs(m, n, k, seed=3)
+    Ad, Bd = dev(A), dev(B)
+    for s in range(1, 9):
+        C = torch.empty((m, n), dtype=torch.float64, device=DEV)
+        dfe.df_emul_gemm_slices(Ad, Bd, C, m, n, k, s)
+        torch.cuda.synchronize()
+        assert np.array_equal(C.cpu().numpy(), O.emul_gemm(A, B, s)), f"s={s}"
+    assert dfe.df_last_status() == 0
+
+
+def test_emul_gemm_two_flush_chunks_bitwise(dfe, gpu_ws):
+    m, n, k, s = 130, 70, 16352 + 1500, 8
+    A, B = G.make_gemm_inputs(m, n, k, seed=8)
+    C = torch.empty((m, n), dtype=torch.float64, device=DEV)
+    dfe.df_emul_gemm_slices(dev(A), dev(B), C, m, n, k, s)
+    torch.cuda.synchronize()
+    assert np.array_equal(C.cpu().numpy(), O.emul_gemm(A, B, s))
+
+
+@pytest.mark.parametrize("tol", TOLS)
+def test_emul_gemm_within_tol(dfe, gpu_ws, tol):
+    m, n, k = 512, 384, 2048
+    A, B = G.make_gemm_inputs(m, n, k, seed=4)
+    C = torch.empty((m, n), dtype=torch.float64, device=DEV)
+    dfe.df_emul_gemm(dev(A), dev(B), C, m, n, k, tol)
+    torch.cuda.synchronize()
+    err = O.rel_frobenius(C.cpu().numpy(), O.gemm_plain(A, B))
+    assert err <= tol, (err, tol, dfe.df_slices_for_tol(tol))
+
+
+def test_emul_gemm_max_slices_1e12(dfe, gpu_ws):
+    m, n, k = 256, 256, 1024
+    A, B = G.make_gemm_inputs(m, n, k, seed=5)
+    C = torch.empty((m, n), dtype=torch.float64, device=DEV)
+    dfe.df_emul_gemm_slices(dev(A), dev(B), C, m, n, k, 8)
+    torch.cuda.synchronize()
+    ref = O.gemm_longdouble(A, B)
+    err = float(np.linalg.norm((C.cpu().numpy() - ref).astype(np.float64)) / np.linalg.norm(ref.astype(np.float64)))
+    assert err <= 1e-12, err
+
+
+def test_emul_gemm_zero_and_degenerate(dfe, gpu_ws):
+    A = np.zeros((40, 50)); B = np.random.default_rng(0).standard_normal((50, 30))
+    C = torch.full((40, 30), 7.0, dtype=torch.float64, device=DEV)
+    dfe.df_emul_gemm_slices(dev(A), dev(B), C, 40, 30, 50, 4)
+    torch.cuda.synchronize()
+    assert not C.cpu().numpy().any()
+    with pytest.raises(dfe.DFError):
+        dfe.df_emul_gemm_slices(dev(A), dev(B), C, 0, 30, 50, 4)  # empty input is an argument error
+
+
+def run_jk(dfe, Bp, cfg_nao, naux, Cocc, nocc, D, s, want_x=True):
+    a_pad = (nocc + 15) // 16 * 16
+    J = torch.empty((cfg_nao, cfg_nao), dtype=torch.float64, device=DEV)
+    K = torch.empty_like(J)
+    X = torch.zeros((cfg_nao, naux, a_pad), dtype=torch.float64, device=DEV) if want_x else None
+    e6 = torch.zeros((4096, cfg_nao), dtype=torch.int32, device=DEV)
+    ng = dfe.df_debug_jk_build(dev(Bp), cfg_nao, naux, dev(Cocc), nocc, dev(D), s, J, K, X, e6)
+    torch.cuda.synchronize()
+    return J.cpu().numpy(), K.cpu().numpy(), (X.cpu().numpy() if want_x else None), e6.cpu().numpy()[:ng], ng
+
+
+@pytest.mark.parametrize("tol", [1e-4, 1e-8, 1e-12])
+def test_jk_tiny_config0(dfe, gpu_ws, tol):
+    cfg = G.CONFIGS["tiny"]
+    Bp, Cocc, D = G.make_df_inputs(cfg)
+    s = dfe.df_slices_for_tol(tol)
+    J, K, X, e6, ng = run_jk(dfe, Bp, cfg.nao, cfg.naux, Cocc, cfg.nocc, D, s)
+    J_ref, K_ref = O.df_jk_plain(Bp, cfg.nao, Cocc, D)
+    K_emu, X_emu = O.emul_df_k(Bp, cfg.nao, Cocc, s, return_x=True)
+    assert O.rel_frobenius(J, J_ref) <= 1e-12
+    assert O.rel_frobenius(K, K_ref) <= tol
+    # stage by stage: GEMM(5) output bit-exact, GEMM(6) scales exact, K up to FP64 summation order
+    assert np.array_equal(X[:, :, :cfg.nocc].transpose(1, 0, 2), X_emu)
+    assert not X[:, :, cfg.nocc:].any()
+    groups = O.q_groups(cfg.naux, cfg.nocc, s)
+    assert ng == len(groups)
+    for g, (g0, g1) in enumerate(groups):
+        Xrow = np.transpose(X_emu[g0:g1], (1, 0, 2)).reshape(cfg.nao, -1)
+        assert np.array_equal(e6[g], O.scale_index(np.max(np.abs(Xrow), axis=1)))
+    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert np.array_equal(J, J.T) and np.array_equal(K, K.T)
+    assert np.linalg.eigvalsh(K).min() >= -1e-12 * np.abs(K).max()
+    assert dfe.df_last_status() == 0
+    # the same call through the tol entry point gives the same bits
+    J2 = torch.empty((cfg.nao, cfg.nao), dtype=torch.float64, device=DEV); K2 = torch.empty_like(J2)
+    dfe.df_jk_build(dev(Bp), cfg.nao, cfg.naux, dev(Cocc), cfg.nocc, dev(D), tol, J2, K2)
+    torch.cuda.synchronize()
+    assert np.array_equal(K2.cpu().numpy(), K)
+
+
+def test_jk_many_groups_and_superblocks(dfe, gpu_ws):
+    """naux spans three 512-blocks (ragged last one), two q-groups per block, ragged nao/nocc;
+    a minimum-size workspace forces one super-block per 512 q and must give the same bits."""
+    nao, naux, nocc, s = 40, 1100, 40, 8
+    Bp = G.make_B_packed(nao, naux, seed=7)
+    Cocc = G.make_C_occ(nao, nocc, seed=7)
+    D = G.make_density(Cocc)
+    groups = O.q_groups(naux, nocc, s)
+    assert len(groups) == 6
+    J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+    K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
+    J_ref, K_ref = O.df_jk_plain(Bp, nao, Cocc, D)
+    assert ng == 6
+    assert np.array_equal(X[:, :, :nocc].transpose(1, 0, 2), X_emu)
+    for g, (g0, g1) in enumerate(groups):
+        Xrow = np.transpose(X_emu[g0:g1], (1, 0, 2)).reshape(nao, -1)
+        assert np.array_equal(e6[g], O.scale_index(np.max(np.abs(Xrow), axis=1)))
+    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert O.rel_frobenius(K, K_ref) <= 1e-12 and O.rel_frobenius(J, J_ref) <= 1e-12
+    small = dfe.Workspace(dfe.df_jk_workspace_bytes(nao, naux, nocc, s))
+    try:
+        J2, K2, X2, e62, ng2 = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+    finally:
+        small.close()
+        dfe.df_set_workspace(gpu_ws.view)
+    assert ng2 == 6 and np.array_equal(K2, K) and np.array_equal(X2, X) and np.array_equal(J2, J)
+
+
+def test_jk_workspace_too_small(dfe, gpu_ws):
+    tiny = dfe.Workspace(4096)
+    try:
+        with pytest.raises(dfe.DFError) as ei:
+            run_jk(dfe, *G.make_df_inputs(G.CONFIGS["tiny"])[:1], 48, 160, np.zeros((48, 10)), 10, np.zeros((48, 48)), 3)
+        assert ei.value.code == -4
+    finally:
+        tiny.close()
+        dfe.df_set_workspace(gpu_ws.view)
+
+
+def test_jk_naux_1_rank_one(dfe, gpu_ws):
+    """naux = 1: J = (b.d) b and K = (B C)(B C)^T, the textbook special case."""
+    nao, nocc = 33, 7
+    Bp = G.make_B_packed(nao, 1, seed=9)
+    Cocc = G.make_C_occ(nao, nocc, seed=9)
+    D = G.make_density(Cocc)
+    J, K, _, _, ng = run_jk(dfe, Bp, nao, 1, Cocc, nocc, D, 8)
+    Bm = O.unpack_sym(Bp[:, 0], nao)
+    assert ng == 1
+    assert np.allclose(J, np.sum(Bm * D) * Bm, rtol=1e-12, atol=1e-14 * np.abs(Bm).max())
+    assert O.rel_frobenius(K, (Bm @ Cocc) @ (Bm @ Cocc).T) <= 1e-12
