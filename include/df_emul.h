@@ -154,6 +154,10 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
                       int s, double* J, double* K,
                       double* X_out, int32_t* e6_out, int* ngroups_out, void* stream);
 
+/* Timing experiments on the GEMM kernel (results are then garbage): bit 0 = issue no
+ * MMAs (operand feed only), bit 1 = issue no TMA loads (MMA issue only).  0 = normal. */
+int df_debug_set_gemm_flags(int flags);
+
 /* Number of GPU kernels this library has launched in this process. */
 int64_t df_launch_count(void);
 

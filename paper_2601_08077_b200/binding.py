@@ -56,6 +56,7 @@ _SIG = {
     "df_debug_weight_sums": (_i32, [_vp, _vp, _i64, _i64, _i64, _i32, _i32, _i32, _vp, _vp]),
     "df_debug_jk_build": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp, _vp,
                                  C.POINTER(C.c_int), _vp]),
+    "df_debug_set_gemm_flags": (_i32, [_i32]),
     "df_launch_count": (_i64, []),
     "df_profile_enable": (_i32, [_i32]),
     "df_profile_num_classes": (_i32, []),
@@ -220,6 +221,10 @@ def df_debug_jk_build(B_packed, nao, naux, C_occ, nocc, D, s, J, K, X_out=None, 
                                  _ptr(e6_out, torch.int32) if e6_out is not None else None,
                                  C.byref(ng), _stream(stream)), "df_debug_jk_build")
     return int(ng.value)
+
+
+def df_debug_set_gemm_flags(flags: int) -> None:
+    _check(lib.df_debug_set_gemm_flags(int(flags)), "df_debug_set_gemm_flags")
 
 
 def df_launch_count() -> int:

@@ -248,7 +248,7 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
                    int s, double* J, double* K, double* X_out, int32_t* e6_out, int* ngroups_out,
                    cudaStream_t st) {
   if (!Bp || !Cocc || !D || !J || !K) return DF_ERR_NULL;
-  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nao > 8160 || naux > (1 << 20)) return DF_ERR_DIM;
+  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nao > 11552 || naux > (1 << 20)) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
   if (!device_ok()) return DF_ERR_DEVICE;
   if (!g_ws) return DF_ERR_WORKSPACE;
@@ -546,6 +546,11 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t 
   g.P = P;
   g.dbg_chunk = chunk;
   if (launch_gemm_i8(g, (cudaStream_t)stream) != cudaSuccess) return DF_ERR_CUDA;
+  return DF_OK;
+}
+
+int df_debug_set_gemm_flags(int flags) {
+  set_gemm_debug_flags(flags);
   return DF_OK;
 }
 

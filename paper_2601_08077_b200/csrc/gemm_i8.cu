@@ -24,7 +24,7 @@ namespace dfe {
 
 constexpr int kMaxStages = 8;
 constexpr int kGemmThreads = 192;
-constexpr int kSmemLimit = 232448;  // 227 KB
+constexpr int kSmemLimit = 232448 - 19456;  // 227 KB minus the static shared memory (barriers, epilogue staging)
 
 struct GemmKernelParams {
   CUtensorMap mapA;
@@ -49,6 +49,12 @@ struct GemmKernelParams {
   uint32_t* xmax;
   int32_t* P;
   int dbg_chunk;
+  // flattened slice-pair list: x = A plane offset>>4 | (B plane offset>>4) << 16 within a stage,
+  // y = accumulator column | (accumulate-from-the-start flag) << 16; pass ps owns
+  // [pass_start[ps], pass_start[ps+1])
+  uint2 pairs[kMaxSlices * (kMaxSlices + 1) / 2];
+  int pass_start[kMaxSlices + 1];
+  int dbg_flags;  // bit 0: no MMAs (operand feed only); bit 1: no TMA loads (MMA issue only)
 };
 
 // weights of pass `ps`: w_hi down to w_lo
@@ -81,7 +87,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   __shared__ __align__(8) uint64_t tmem_full_bar;
   __shared__ __align__(8) uint64_t tmem_empty_bar;
   __shared__ uint32_t tmem_slot;
-  __shared__ uint4 pair_tab[kMaxSlices * (kMaxSlices + 1) / 2];
+  __shared__ __align__(16) double epi_stage[4][32][18];  // per epilogue warp: 32 rows x 16 cols, 144 B pitch
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -138,6 +144,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             const uint32_t stage = it % S;
             const uint32_t ph = (it / S) & 1u;
             mbar_wait(&empty_bar[stage], ph ^ 1u);
+            if (p.dbg_flags & 2) {
+              mbar_arrive(&full_bar[stage]);
+              continue;
+            }
             uint8_t* st = smem + (size_t)stage * p.stage_stride;
             mbar_expect_tx(&full_bar[stage], tx);
             const int kpos = kc0 + kb * BK;
@@ -151,59 +161,57 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     }
   } else if (warp == 1) {
     // ================= MMA issuer =================
-    // One thread issues every MMA, so the per-MMA instruction count must stay far below the
-    // MMA's own duration (64 cycles at N = 128): the (t, u, w) loop nest is flattened once per
-    // pass into a table {A plane offset, B plane offset, accumulator column, accumulate flag},
-    // and the inner loop only adds the K offset to the descriptors' address fields.
-    if (lane == 0) {
-      const uint32_t idesc = make_idesc_i8(kTileM, p.n_tile);
-      const uint64_t desc_proto = make_smem_desc(0, BK);
-      const uint32_t desc_hi = (uint32_t)(desc_proto >> 32);
-      const uint32_t desc_lo0 = (uint32_t)desc_proto;  // LBO field, address 0
-      uint32_t it = 0, iter = 0;
-      for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
-        const int kc0 = zk0 + ch * p.kflush;
-        const int kc1 = min(zk1, kc0 + p.kflush);
-        const int nkb = (kc1 - kc0 + BK - 1) / BK;
-        for (int ps = 0; ps < npass; ++ps, ++iter) {
-          int w_hi, w_lo;
-          pass_weights(s, W, ps, w_hi, w_lo);
-          int np = 0;
-          for (int w = w_hi; w >= w_lo; --w) {
-            const int t_lo = max(1, w - s), t_hi = min(s, w - 1);
-            for (int t = t_lo; t <= t_hi; ++t, ++np)
-              pair_tab[np] = make_uint4(((uint32_t)(t - 1) * a_plane_bytes) >> 4,
-                                        (b_off + (uint32_t)(w - t - 1) * b_plane_bytes) >> 4,
-                                        tmem_base + (uint32_t)((w_hi - w) * p.acc_stride), t > t_lo ? 1u : 0u);
+    // The whole warp runs this loop with warp-uniform control flow and one elected lane issues,
+    // so descriptors live in uniform registers.  The (w, t, u) nest is flattened on the host into
+    // p.pairs (constant bank): per MMA the loop adds two 16-bit offsets to the descriptor address
+    // field -- far fewer issue cycles than the MMA's own 64+ cycles.
+    const uint32_t idesc = make_idesc_i8(kTileM, p.n_tile);
+    const uint64_t desc_proto = make_smem_desc(0, BK);
+    const uint32_t desc_hi = (uint32_t)(desc_proto >> 32);
+    const uint32_t desc_lo0 = (uint32_t)desc_proto;  // LBO field, address 0
+    const uint32_t smem_base16 = (smem_u32(smem) & 0x3FFFFu) >> 4;
+    const uint32_t stage16 = p.stage_stride >> 4;
+    uint32_t it = 0, iter = 0;
+    for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
+      const int kc0 = zk0 + ch * p.kflush;
+      const int kc1 = min(zk1, kc0 + p.kflush);
+      const int nkb = (kc1 - kc0 + BK - 1) / BK;
+      for (int ps = 0; ps < npass; ++ps, ++iter) {
+        const int pr0 = p.pass_start[ps], pr1 = p.pass_start[ps + 1];
+        if (iter > 0) {
+          mbar_wait(&tmem_empty_bar, (iter - 1) & 1u);
+          tc_fence_after();
+        }
+        for (int kb = 0; kb < nkb; ++kb, ++it) {
+          const uint32_t stage = it % S;
+          const uint32_t ph = (it / S) & 1u;
+          mbar_wait(&full_bar[stage], ph);
+          tc_fence_after();
+          if (p.dbg_flags & 1) {
+            if (lane == 0) mbar_arrive(&empty_bar[stage]);
+            continue;
           }
-          if (iter > 0) {
-            mbar_wait(&tmem_empty_bar, (iter - 1) & 1u);
-            tc_fence_after();
-          }
-          for (int kb = 0; kb < nkb; ++kb, ++it) {
-            const uint32_t stage = it % S;
-            const uint32_t ph = (it / S) & 1u;
-            mbar_wait(&full_bar[stage], ph);
-            tc_fence_after();
-            const uint32_t sa = smem_u32(smem + (size_t)stage * p.stage_stride);
-            const uint32_t lo_base = desc_lo0 | ((sa & 0x3FFFFu) >> 4);
-            const int kpos = kc0 + kb * BK;
-            const int nkk = (min(BK, kc1 - kpos) + 31) / 32;
+          const uint32_t lo_base = desc_lo0 | (smem_base16 + stage * stage16);
+          const int kpos = kc0 + kb * BK;
+          const int nkk = (min(BK, kc1 - kpos) + 31) / 32;
+          if (elect_one()) {
             for (int kk = 0; kk < nkk; ++kk) {
               const uint32_t lo = lo_base + 2u * kk;  // +32 bytes per K step, in 16-byte units
               const uint32_t later = (kb | kk) ? 1u : 0u;
-#pragma unroll 4
-              for (int i = 0; i < np; ++i) {
-                const uint4 e = pair_tab[i];
-                const uint64_t adesc = ((uint64_t)desc_hi << 32) | (lo + e.x);
-                const uint64_t bdesc = ((uint64_t)desc_hi << 32) | (lo + e.y);
-                mma_i8_ss(e.z, adesc, bdesc, idesc, later | e.w);
+#pragma unroll 2
+              for (int i = pr0; i < pr1; ++i) {
+                const uint2 e = p.pairs[i];
+                const uint64_t adesc = ((uint64_t)desc_hi << 32) | (lo + (e.x & 0xFFFFu));
+                const uint64_t bdesc = ((uint64_t)desc_hi << 32) | (lo + (e.x >> 16));
+                mma_i8_ss(tmem_base + (e.y & 0xFFFFu), adesc, bdesc, idesc, later | (e.y >> 16));
               }
             }
             mma_commit(&empty_bar[stage]);  // frees the smem stage once these MMAs have read it
           }
-          mma_commit(&tmem_full_bar);  // accumulators of this pass are complete
+          __syncwarp();
         }
+        if (elect_one()) mma_commit(&tmem_full_bar);  // accumulators of this pass are complete
+        __syncwarp();
       }
     }
   } else {
@@ -223,6 +231,26 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
       const long long q = row / p.nao;
       const long long i = row - q * p.nao;
       out = p.C + i * p.ldx + q * p.n_tile - col0;  // col0 == 0 in this mode
+    }
+    // coalesced phase: lane moves columns cpair, cpair+1 of rows (lane >> 3) + 4 j, j = 0..7
+    const int cpair = (lane & 7) * 2;
+    double(*stg)[18] = epi_stage[quarter];
+    double* srow[8];
+    const long long ld_out = (p.mode == kEpiX) ? p.ldx : p.ldc;
+    const bool vec_ok = p.mode != kEpiInt32 && ((ld_out | p.c_stride | (long long)col0) & 1) == 0 &&
+                        ((uintptr_t)p.C & 15) == 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const long long rr = (long long)tm * kTileM + quarter * 32 + (lane >> 3) + 4 * j;
+      srow[j] = nullptr;
+      if (rr < p.a_rows) {
+        if (p.mode == kEpiC) {
+          srow[j] = p.C + z * p.c_stride + rr * p.ldc;
+        } else if (p.mode == kEpiX) {
+          const long long q = rr / p.nao;
+          srow[j] = p.C + (rr - q * p.nao) * p.ldx + q * p.n_tile - col0;
+        }
+      }
     }
     uint32_t iter = 0;
     uint32_t hi_max = 0;
@@ -255,9 +283,36 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
 #pragma unroll
           for (int j = 0; j < 16; ++j) {
             const long long col = col0 + c + j;
-            const bool ok = row_ok && col < p.b_rows;
-            eBv[j] = ok ? p.eB[z * p.eb_stride + col] : 0;
-            acc[j] = (ok && !first) ? out[col] : 0.0;
+            eBv[j] = (row_ok && col < p.b_rows) ? p.eB[z * p.eb_stride + col] : 0;
+            acc[j] = 0.0;
+          }
+          const long long colv = col0 + c + cpair;  // first of the two columns this lane moves
+          if (!first) {
+            // running sum of the earlier passes/chunks: coalesced 16-byte loads (8 lanes cover one
+            // row's 128 bytes), transposed through shared memory to "lane = row"
+            if (vec_ok) {
+#pragma unroll
+              for (int j = 0; j < 8; ++j) {
+                double2 v = make_double2(0.0, 0.0);
+                if (srow[j] && colv + 1 < p.b_rows) v = *reinterpret_cast<const double2*>(srow[j] + colv);
+                else if (srow[j] && colv < p.b_rows) v.x = srow[j][colv];
+                *reinterpret_cast<double2*>(&stg[(lane >> 3) + 4 * j][cpair]) = v;
+              }
+              __syncwarp();
+#pragma unroll
+              for (int j = 0; j < 8; ++j) {
+                const double2 v = *reinterpret_cast<const double2*>(&stg[lane][2 * j]);
+                acc[2 * j] = v.x;
+                acc[2 * j + 1] = v.y;
+              }
+              __syncwarp();
+            } else {
+#pragma unroll
+              for (int j = 0; j < 16; ++j) {
+                const long long col = col0 + c + j;
+                if (row_ok && col < p.b_rows) acc[j] = out[col];
+              }
+            }
           }
           for (int w = w_hi; w >= w_lo; --w) {
             tmem_ld16(t_lane + (uint32_t)((w_hi - w) * p.acc_stride + c), v);
@@ -267,12 +322,28 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             for (int j = 0; j < 16; ++j)
               acc[j] = fma((double)(int32_t)v[j], pow2_double(eb + eBv[j]), acc[j]);
           }
+          if (last && row_ok) {
 #pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const long long col = col0 + c + j;
-            if (row_ok && col < p.b_rows) {
-              out[col] = acc[j];
-              if (last) hi_max = max(hi_max, abs_hi_word(acc[j]));
+            for (int j = 0; j < 16; ++j)
+              if (col0 + c + j < p.b_rows) hi_max = max(hi_max, abs_hi_word(acc[j]));
+          }
+          if (vec_ok) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+              *reinterpret_cast<double2*>(&stg[lane][2 * j]) = make_double2(acc[2 * j], acc[2 * j + 1]);
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const double2 v = *reinterpret_cast<const double2*>(&stg[(lane >> 3) + 4 * j][cpair]);
+              if (srow[j] && colv + 1 < p.b_rows) *reinterpret_cast<double2*>(srow[j] + colv) = v;
+              else if (srow[j] && colv < p.b_rows) srow[j][colv] = v.x;
+            }
+            __syncwarp();
+          } else {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+              const long long col = col0 + c + j;
+              if (row_ok && col < p.b_rows) out[col] = acc[j];
             }
           }
         }
@@ -393,18 +464,28 @@ static uint32_t stage_stride_for(int s, int n_tile, int bk) {
   return (uint32_t)round_up((int64_t)s * (kTileM + n_tile) * bk, 1024);
 }
 
+static int g_gemm_dbg_flags = 0;
+static int g_gemm_force_bk = 0;
+void set_gemm_debug_flags(int flags) {
+  g_gemm_dbg_flags = flags & 3;
+  const int f = (flags >> 8) & 0xFF;  // bits 8..15: force the K-block width (32, 64, 128; 0 = auto)
+  g_gemm_force_bk = (f == 32 || f == 64 || f == 128) ? f : 0;
+}
+
 cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   GemmKernelParams p;
   const int s = g.s;
   int bk = g.bk;
+  if (bk == 0) bk = g_gemm_force_bk;
   if (bk == 0) {
-    bk = 32;
-    for (int cand = 128; cand >= 32; cand /= 2)
-      if ((kSmemLimit - 2048) / (int)stage_stride_for(s, g.n_tile, cand) >= 3) {
-        bk = cand;
-        break;
-      }
+    // widest swizzle span that still gives three stages; failing that, two 64-byte stages
+    auto stages = [&](int cand) { return (kSmemLimit - 2048) / (int)stage_stride_for(s, g.n_tile, cand); };
+    if (stages(128) >= 3) bk = 128;
+    else if (stages(64) >= 2) bk = 64;
+    else bk = 32;
   }
+  // a forced K-block width that leaves no room for even one stage is narrowed
+  while (bk > 32 && (kSmemLimit - 2048) / (int)stage_stride_for(s, g.n_tile, bk) < 1) bk /= 2;
   p.stage_stride = stage_stride_for(s, g.n_tile, bk);
   p.num_stages = (int)((kSmemLimit - 2048) / p.stage_stride);
   if (p.num_stages > kMaxStages) p.num_stages = kMaxStages;
@@ -417,6 +498,24 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.acc_stride = (int)round_up(g.n_tile, 32);
   p.weights_per_pass = 512 / p.acc_stride;
   if (p.weights_per_pass > s) p.weights_per_pass = s;
+  {
+    const int W = p.weights_per_pass, npass = (s + W - 1) / W;
+    const uint32_t a_plane = (uint32_t)kTileM * bk, b_plane = (uint32_t)g.n_tile * bk, b_off = (uint32_t)s * a_plane;
+    int np = 0;
+    for (int ps = 0; ps < npass; ++ps) {
+      p.pass_start[ps] = np;
+      const int w_hi = s + 1 - ps * W, w_lo = (w_hi - W + 1) > 2 ? (w_hi - W + 1) : 2;
+      for (int w = w_hi; w >= w_lo; --w) {
+        const int t_lo = (w - s) > 1 ? (w - s) : 1, t_hi = (w - 1) < s ? (w - 1) : s;
+        for (int t = t_lo; t <= t_hi; ++t, ++np) {
+          const uint32_t ao = ((uint32_t)(t - 1) * a_plane) >> 4, bo = (b_off + (uint32_t)(w - t - 1) * b_plane) >> 4;
+          p.pairs[np].x = ao | (bo << 16);
+          p.pairs[np].y = (uint32_t)((w_hi - w) * p.acc_stride) | ((t > t_lo ? 1u : 0u) << 16);
+        }
+      }
+    }
+    p.pass_start[npass] = np;
+  }
   p.tiles_m = (int)((g.a_rows + kTileM - 1) / kTileM);
   p.tiles_n = (int)((g.b_rows + g.n_tile - 1) / g.n_tile);
   p.group_m = 16;
@@ -440,6 +539,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.xmax = g.xmax;
   p.P = g.P;
   p.dbg_chunk = g.dbg_chunk;
+  p.dbg_flags = g_gemm_dbg_flags;
 
   const size_t smem = (size_t)p.num_stages * p.stage_stride + 1024;
   dim3 grid((unsigned)((int64_t)p.tiles_m * p.tiles_n), 1, (unsigned)g.nz);

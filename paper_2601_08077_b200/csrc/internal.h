@@ -63,6 +63,7 @@ struct GemmProblem {
 };
 
 cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st);
+void set_gemm_debug_flags(int flags);
 cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStream_t st);
 
 // ---- jk.cu ----------------------------------------------------------------

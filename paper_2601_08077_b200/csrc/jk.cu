@@ -21,11 +21,9 @@
 
 namespace dfe {
 
-// block index -> (row tile TR, column tile TC) of the full square; returns false for the unused
-// mirror of a diagonal tile.
-__device__ __forceinline__ bool tile_of_block(unsigned bx, int& TR, int& TC, bool& lower) {
-  const unsigned idx = bx >> 1;
-  const int flip = bx & 1;
+// (tile pair index, flip) -> (row tile TR, column tile TC) of the full square; returns false for
+// the unused mirror of a diagonal tile.  Pair idx = a(a+1)/2 + b, a >= b.
+__device__ __forceinline__ bool tile_of_block(unsigned idx, int flip, int& TR, int& TC, bool& lower) {
   int a = (int)((sqrtf(8.0f * (float)idx + 1.0f) - 1.0f) * 0.5f);
   while ((unsigned)(a + 1) * (unsigned)(a + 2) / 2 <= idx) ++a;
   while ((unsigned)a * (unsigned)(a + 1) / 2 > idx) --a;
@@ -37,6 +35,21 @@ __device__ __forceinline__ bool tile_of_block(unsigned bx, int& TR, int& TC, boo
   return true;
 }
 
+// Walks the packed rows p(R, C) for C = C0, C0+1, ...: consecutive rows while C <= R, then a
+// stride of C+1 rows (p(C, R) = C(C+1)/2 + R).
+struct PackedRowWalker {
+  long long p;
+  int R, C;
+  __device__ __forceinline__ PackedRowWalker(int R_, int C0) : R(R_), C(C0) {
+    const long long hi = max(R_, C0), lo = min(R_, C0);
+    p = hi * (hi + 1) / 2 + lo;
+  }
+  __device__ __forceinline__ void next() {
+    p += (C < R) ? 1 : (C + 1);
+    ++C;
+  }
+};
+
 __device__ __forceinline__ long long packed_row(int R, int C) {
   const long long hi = max(R, C), lo = min(R, C);
   return hi * (hi + 1) / 2 + lo;
@@ -47,9 +60,11 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
                                                         uint32_t* __restrict__ emax) {
   int TR, TC;
   bool lower;
-  if (!tile_of_block(blockIdx.y, TR, TC, lower)) return;
+  // blockIdx.x = 2 * q-chunk + flip: a tile and its mirror read the same 256 KB back to back (the
+  // second read is an L2 hit) and neighbouring blocks read adjacent 256-byte runs of the same rows
+  if (!tile_of_block(blockIdx.y, blockIdx.x & 1, TR, TC, lower)) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = blockIdx.x * 32 + lane;  // q chunk fastest: concurrent blocks read adjacent runs of a row
+  const int q = (blockIdx.x >> 1) * 32 + lane;
   const bool q_ok = q < naux;
   __shared__ double rho_sh[8][32];
   double rsum = 0.0;
@@ -58,10 +73,12 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
     if (R >= nao) break;
     uint32_t hm = 0;
     const int c_end = min(32, nao - TC * 32);
+    PackedRowWalker wk(R, TC * 32);
+    const double* bq = Bp + (q_ok ? q : 0);
 #pragma unroll 8
-    for (int cc = 0; cc < c_end; ++cc) {
+    for (int cc = 0; cc < c_end; ++cc, wk.next()) {
       const int C = TC * 32 + cc;
-      const double x = q_ok ? __ldg(Bp + packed_row(R, C) * naux + q) : 0.0;
+      const double x = q_ok ? __ldg(bq + wk.p * naux) : 0.0;
       hm = max(hm, abs_hi_word(x));
       if (lower && C <= R) {
         const double d = 0.5 * (__ldg(D + (long long)R * nao + C) + __ldg(D + (long long)C * nao + R));
@@ -103,9 +120,9 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
                                                               int* __restrict__ status) {
   int TR, TC;
   bool lower;
-  if (!tile_of_block(blockIdx.y, TR, TC, lower)) return;
+  if (!tile_of_block(blockIdx.y, blockIdx.x & 1, TR, TC, lower)) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = q0 + blockIdx.x * 32 + lane;
+  const int q = q0 + (blockIdx.x >> 1) * 32 + lane;
   if (q >= q1) return;
   for (int rr = 0; rr < 4; ++rr) {
     const int R = TR * 32 + warp + 8 * rr;
@@ -124,10 +141,12 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
     for (int t = 0; t < S; ++t)
 #pragma unroll
       for (int j = 0; j < 8; ++j) w[t][j] = 0;
+    PackedRowWalker wk(R, TC * 32);
+    const double* bq = Bp + q;
 #pragma unroll
-    for (int cc = 0; cc < 32; ++cc) {
+    for (int cc = 0; cc < 32; ++cc, wk.next()) {
       const int C = TC * 32 + cc;
-      const double x = (C < nao) ? __ldg(Bp + packed_row(R, C) * naux + q) : 0.0;
+      const double x = (C < nao) ? __ldg(bq + wk.p * naux) : 0.0;
       const uint64_t dg = balanced_digits(x, scale);
 #pragma unroll
       for (int t = 0; t < S; ++t) w[t][cc >> 2] |= digit_byte(dg, t) << (8 * (cc & 3));
@@ -217,14 +236,14 @@ __global__ void __launch_bounds__(256) jk_j_unpack_kernel(const double* __restri
 }
 
 // ---------------------------------------------------------------------------
-static unsigned tile_blocks(int nao) {
+static unsigned tile_pairs(int nao) {
   const unsigned T = (unsigned)((nao + 31) / 32);
-  return T * (T + 1);  // 2 * T(T+1)/2
+  return T * (T + 1) / 2;
 }
 
 cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho, uint32_t* emax,
                              cudaStream_t st) {
-  dim3 grid((unsigned)((naux + 31) / 32), tile_blocks(nao));
+  dim3 grid(2u * (unsigned)((naux + 31) / 32), tile_pairs(nao));
   jk_pass_a_kernel<<<grid, 256, 0, st>>>(Bp, nao, naux, D, rho, emax);
   count_launch();
   return cudaGetLastError();
@@ -252,7 +271,7 @@ cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const do
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
                                    int* status, cudaStream_t st) {
-  dim3 grid((unsigned)((q1 - q0 + 31) / 32), tile_blocks(nao));
+  dim3 grid(2u * (unsigned)((q1 - q0 + 31) / 32), tile_pairs(nao));
   DFE_DISPATCH_S(s, (jk_unpack_split_kernel<SS><<<grid, 256, 0, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5,
                                                                       pitch, plane_stride, status)));
   count_launch();
