@@ -20,6 +20,7 @@ static void* g_ws = nullptr;
 static int64_t g_ws_bytes = 0;
 static int g_mode = DF_MODE_GUARDED;
 static int g_device_ok = -1;
+static int g_g5_split_n = 1;
 
 // ---- optional per-kernel-class CUDA-event timing (df_profile_*; bench.py's roofline) ----
 enum ProfClass { kPSplit = 0, kPPassA, kPJGemv, kPUnpack, kPGemm5, kPSplitX, kPGemm6, kPReduce, kPGemm, kPNum };
@@ -326,7 +327,12 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     g5.a_plane_stride = (int64_t)nq * nao * w.pitchj;
     g5.b_plane_stride = (int64_t)w.a_pad * w.pitchj;
     g5.s = s;
+    // N tile: the whole a_pad when all s weight accumulators fit TMEM (s * a_pad <= 512 columns),
+    // else half of it, so that X is written once instead of read-modify-written per pass
     g5.n_tile = w.a_pad;
+    if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) g5.n_tile = w.a_pad / 2;
+    g5.acc_stride = (g5.n_tile % 32) ? g5.n_tile : 0;
+    g5.x_cols = w.a_pad;
     g5.nz = 1;
     g5.eA = w.e5;
     g5.eB = w.eC;
@@ -551,6 +557,7 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t 
 
 int df_debug_set_gemm_flags(int flags) {
   set_gemm_debug_flags(flags);
+  g_g5_split_n = (flags & 4) ? 0 : 1;  // bit 2: GEMM(5) keeps one N tile (multi-pass read-modify-write)
   return DF_OK;
 }
 

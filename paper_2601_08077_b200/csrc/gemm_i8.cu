@@ -43,7 +43,7 @@ struct GemmKernelParams {
   int lower_only, mode;
   double* C;
   long long ldc, c_stride;
-  int nao;
+  int nao, x_cols;
   long long ldx;
   const int* qgroup;
   uint32_t* xmax;
@@ -230,7 +230,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     } else if (p.mode == kEpiX) {
       const long long q = row / p.nao;
       const long long i = row - q * p.nao;
-      out = p.C + i * p.ldx + q * p.n_tile - col0;  // col0 == 0 in this mode
+      out = p.C + i * p.ldx + q * p.x_cols;  // indexed by the global column
     }
     // coalesced phase: lane moves columns cpair, cpair+1 of rows (lane >> 3) + 4 j, j = 0..7
     const int cpair = (lane & 7) * 2;
@@ -248,7 +248,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
           srow[j] = p.C + z * p.c_stride + rr * p.ldc;
         } else if (p.mode == kEpiX) {
           const long long q = rr / p.nao;
-          srow[j] = p.C + (rr - q * p.nao) * p.ldx + q * p.n_tile - col0;
+          srow[j] = p.C + (rr - q * p.nao) * p.ldx + q * p.x_cols;
         }
       }
     }
@@ -495,7 +495,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
     return cudaErrorInvalidValue;
   p.s = s;
   p.n_tile = g.n_tile;
-  p.acc_stride = (int)round_up(g.n_tile, 32);
+  p.acc_stride = g.acc_stride > 0 ? g.acc_stride : (int)round_up(g.n_tile, 32);
   p.weights_per_pass = 512 / p.acc_stride;
   if (p.weights_per_pass > s) p.weights_per_pass = s;
   {
@@ -534,6 +534,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.ldc = g.ldc;
   p.c_stride = g.c_stride;
   p.nao = g.nao;
+  p.x_cols = g.x_cols;
   p.ldx = g.ldx;
   p.qgroup = g.qgroup;
   p.xmax = g.xmax;

@@ -51,9 +51,11 @@ struct GemmProblem {
   // kEpiC: C[z * c_stride + row * ldc + col] (FP64)
   double* C;
   int64_t ldc, c_stride;
-  // kEpiX: row r = (q, i) = (r / nao, r % nao); X[i * ldx + q * n_tile + col]; running max of the
+  // kEpiX: row r = (q, i) = (r / nao, r % nao); X[i * ldx + q * x_cols + col]; running max of the
   // upper word of |X| per (group of q, i): xmax[qgroup[q] * nao + i]
   int nao;
+  int x_cols;       // columns of X per q (a_pad); the N tiles of GEMM(5) cut this range
+  int acc_stride;   // TMEM columns between weight accumulators (0 = n_tile rounded up to 32)
   int64_t ldx;
   const int* qgroup;
   uint32_t* xmax;

@@ -67,22 +67,40 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
   const int q = (blockIdx.x >> 1) * 32 + lane;
   const bool q_ok = q < naux;
   __shared__ double rho_sh[8][32];
+  __shared__ double dw_sh[32][33];  // weighted density of this tile: (i == j ? 1 : 2) * 0.5 (D_ij + D_ji), 0 above the diagonal
+  if (lower) {
+    for (int idx = threadIdx.x; idx < 1024; idx += 256) {
+      const int rl = idx >> 5, cl = idx & 31;
+      const int R = TR * 32 + rl, C = TC * 32 + cl;
+      double v = 0.0;
+      if (R < nao && C <= R) {
+        const double d = 0.5 * (__ldg(D + (long long)R * nao + C) + __ldg(D + (long long)C * nao + R));
+        v = (R == C) ? d : 2.0 * d;
+      }
+      dw_sh[rl][cl] = v;
+    }
+    __syncthreads();
+  }
   double rsum = 0.0;
   for (int rr = 0; rr < 4; ++rr) {
-    const int R = TR * 32 + warp + 8 * rr;
+    const int rl = warp + 8 * rr;
+    const int R = TR * 32 + rl;
     if (R >= nao) break;
     uint32_t hm = 0;
     const int c_end = min(32, nao - TC * 32);
     PackedRowWalker wk(R, TC * 32);
     const double* bq = Bp + (q_ok ? q : 0);
-#pragma unroll 8
-    for (int cc = 0; cc < c_end; ++cc, wk.next()) {
-      const int C = TC * 32 + cc;
-      const double x = q_ok ? __ldg(bq + wk.p * naux) : 0.0;
-      hm = max(hm, abs_hi_word(x));
-      if (lower && C <= R) {
-        const double d = 0.5 * (__ldg(D + (long long)R * nao + C) + __ldg(D + (long long)C * nao + R));
-        rsum = fma((R == C) ? d : 2.0 * d, x, rsum);
+    // 16 loads in flight per thread before the first use (HBM-latency bound otherwise)
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+      double x[16];
+#pragma unroll
+      for (int cc = 0; cc < 16; ++cc, wk.next())
+        x[cc] = (q_ok && half * 16 + cc < c_end) ? __ldg(bq + wk.p * naux) : 0.0;
+#pragma unroll
+      for (int cc = 0; cc < 16; ++cc) {
+        hm = max(hm, abs_hi_word(x[cc]));
+        if (lower) rsum = fma(dw_sh[rl][half * 16 + cc], x[cc], rsum);
       }
     }
     if (q_ok) atomicMax(&emax[(long long)R * naux + q], hm);
@@ -112,48 +130,65 @@ __global__ void __launch_bounds__(256) jk_j_gemv_kernel(const double* __restrict
   if (lane == 0) Jp[p] = acc;
 }
 
+// Unpack + split.  Output planes[t][(q, R)][C] want C-contiguous 128-byte lines, the input wants
+// q-contiguous runs, so: lane <-> q (32 consecutive q, 256-byte loads of one packed row), warp <->
+// one output row R, and the warp walks a whole 128-column block of that row in four 32-column
+// chunks -- every output line is completed by one thread within a few hundred cycles and leaves
+// L2 as a full line.  Blocks are ordered [128 x 128 super-tile pair (A >= B)][q chunk][sub]:
+// sub 0..15 = the 16 row groups of the (A, B) block (rows in A, columns in B), sub 16..31 = the
+// mirrored (B, A) block (rows in B, columns in A).  Both read the same 128 x 128 packed rows of
+// this q chunk (4 MB) back to back, so the second read is an L2 hit.
 template <int S>
 __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __restrict__ Bp, int nao, int naux,
                                                               int q0, int q1, const uint32_t* __restrict__ emax,
                                                               int32_t* __restrict__ e5, int8_t* __restrict__ planes,
                                                               long long pitch, long long plane_stride,
                                                               int* __restrict__ status) {
-  int TR, TC;
+  int A, B;
   bool lower;
-  if (!tile_of_block(blockIdx.y, blockIdx.x & 1, TR, TC, lower)) return;
+  const int sub = blockIdx.x & 31;
+  if (!tile_of_block(blockIdx.y, sub >> 4, A, B, lower)) return;  // (A, B) = (row block, column block)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = q0 + (blockIdx.x >> 1) * 32 + lane;
-  if (q >= q1) return;
-  for (int rr = 0; rr < 4; ++rr) {
-    const int R = TR * 32 + warp + 8 * rr;
-    if (R >= nao) break;
-    const uint32_t hm = emax[(long long)R * naux + q];
-    const int e = scale_index_from_hi(hm);
-    const long long orow = (long long)(q - q0) * nao + R;
-    if (TC == 0) {
-      e5[orow] = e;
-      const int stt = status_from_hi(hm);
-      if (stt) atomicOr(status, stt);
-    }
-    const double scale = pow2_double(63 - e);
+  const int R = A * 128 + (sub & 15) * 8 + warp;
+  const int q = q0 + (blockIdx.x >> 5) * 32 + lane;
+  if (R >= nao || q >= q1) return;
+  const uint32_t hm = emax[(long long)R * naux + q];
+  const int e = scale_index_from_hi(hm);
+  const long long orow = (long long)(q - q0) * nao + R;
+  if (lower && B == 0) {
+    e5[orow] = e;
+    const int stt = status_from_hi(hm);
+    if (stt) atomicOr(status, stt);
+  }
+  const double scale = pow2_double(63 - e);
+  const double* bq = Bp + q;
+  for (int chunk = 0; chunk < 4; ++chunk) {
+    const int C0 = B * 128 + chunk * 32;
+    if (C0 >= pitch) break;
     uint32_t w[S][8];
 #pragma unroll
     for (int t = 0; t < S; ++t)
 #pragma unroll
       for (int j = 0; j < 8; ++j) w[t][j] = 0;
-    PackedRowWalker wk(R, TC * 32);
-    const double* bq = Bp + q;
+    PackedRowWalker wk(R, C0);
+    // all loads of a half chunk are issued before the first conversion (16 requests in flight)
 #pragma unroll
-    for (int cc = 0; cc < 32; ++cc, wk.next()) {
-      const int C = TC * 32 + cc;
-      const double x = (C < nao) ? __ldg(bq + wk.p * naux) : 0.0;
-      const uint64_t dg = balanced_digits(x, scale);
+    for (int half = 0; half < 2; ++half) {
+      double x[16];
 #pragma unroll
-      for (int t = 0; t < S; ++t) w[t][cc >> 2] |= digit_byte(dg, t) << (8 * (cc & 3));
+      for (int cc = 0; cc < 16; ++cc, wk.next())
+        x[cc] = (C0 + half * 16 + cc < nao) ? __ldg(bq + wk.p * naux) : 0.0;
+#pragma unroll
+      for (int cc = 0; cc < 16; ++cc) {
+        const uint64_t dg = balanced_digits(x[cc], scale);
+        const int c32 = half * 16 + cc;
+#pragma unroll
+        for (int t = 0; t < S; ++t) w[t][c32 >> 2] |= digit_byte(dg, t) << (8 * (c32 & 3));
+      }
     }
 #pragma unroll
     for (int t = 0; t < S; ++t) {
-      uint4* dst = reinterpret_cast<uint4*>(planes + t * plane_stride + orow * pitch + TC * 32);
+      uint4* dst = reinterpret_cast<uint4*>(planes + t * plane_stride + orow * pitch + C0);
       dst[0] = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
       dst[1] = make_uint4(w[t][4], w[t][5], w[t][6], w[t][7]);
     }
@@ -271,7 +306,8 @@ cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const do
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
                                    int* status, cudaStream_t st) {
-  dim3 grid(2u * (unsigned)((q1 - q0 + 31) / 32), tile_pairs(nao));
+  const unsigned T128 = (unsigned)((nao + 127) / 128);
+  dim3 grid(32u * (unsigned)((q1 - q0 + 31) / 32), T128 * (T128 + 1) / 2);
   DFE_DISPATCH_S(s, (jk_unpack_split_kernel<SS><<<grid, 256, 0, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5,
                                                                       pitch, plane_stride, status)));
   count_launch();

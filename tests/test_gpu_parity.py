@@ -252,6 +252,26 @@ def test_jk_many_groups_and_superblocks(dfe, gpu_ws):
     assert ng2 == 5 and np.array_equal(K2, K) and np.array_equal(X2, X) and np.array_equal(J2, J)
 
 
+@pytest.mark.parametrize("s", [4, 8])
+def test_jk_split_n_tiles(dfe, gpu_ws, s):
+    """nocc = 150 (config 3's value): a_pad = 160 does not fit s accumulators in TMEM, so GEMM(5)
+    runs two N tiles of 80 columns (s = 4: one pass; s = 8: two passes with the FP64 read-modify-
+    write); ragged nao, several M tiles straddling q boundaries."""
+    nao, naux, nocc = 168, 37, 150
+    Bp = G.make_B_packed(nao, naux, seed=13)
+    Cocc = G.make_C_occ(nao, nocc, seed=13)
+    D = G.make_density(Cocc)
+    J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+    K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
+    J_ref, K_ref = O.df_jk_plain(Bp, nao, Cocc, D)
+    assert np.array_equal(X[:, :, :nocc].transpose(1, 0, 2), X_emu)
+    assert not X[:, :, nocc:].any()
+    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert O.rel_frobenius(J, J_ref) <= 1e-12
+    assert O.rel_frobenius(K, K_ref) <= (1e-6 if s == 4 else 1e-12)
+    assert dfe.df_last_status() == 0
+
+
 def test_jk_workspace_too_small(dfe, gpu_ws):
     tiny = dfe.Workspace(4096)
     try:
