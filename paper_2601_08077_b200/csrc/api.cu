@@ -557,7 +557,8 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t 
 
 int df_debug_set_gemm_flags(int flags) {
   set_gemm_debug_flags(flags);
-  g_g5_split_n = (flags & 4) ? 0 : 1;  // bit 2: GEMM(5) keeps one N tile (multi-pass read-modify-write)
+  g_g5_split_n = (flags & 4) ? 0 : 1;
+  set_jk_debug_flags((flags >> 4) & 3);  // bits 4, 5: unpack kernel without stores / without loads  // bit 2: GEMM(5) keeps one N tile (multi-pass read-modify-write)
   return DF_OK;
 }
 

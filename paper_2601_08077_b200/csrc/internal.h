@@ -68,6 +68,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st);
 void set_gemm_debug_flags(int flags);
 cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStream_t st);
 
+void set_jk_debug_flags(int flags);  // timing experiments: bit 0 = unpack writes nothing, bit 1 = reads nothing
 // ---- jk.cu ----------------------------------------------------------------
 // pass A over packed B: rho[q] (+=, must be zeroed) and emax[i * naux + q] = upper word of
 // max_j |B^q_ij| (atomicMax, must be zeroed).

@@ -130,68 +130,77 @@ __global__ void __launch_bounds__(256) jk_j_gemv_kernel(const double* __restrict
   if (lane == 0) Jp[p] = acc;
 }
 
+// Four consecutive elements' digit words (upper or lower halves) -> the packed plane word of
+// digit byte `b` (0..3 within the half): three byte permutes instead of twelve shift/mask/or.
+__device__ __forceinline__ uint32_t pack4_digit(uint32_t h0, uint32_t h1, uint32_t h2, uint32_t h3, int b) {
+  const uint32_t sel = (uint32_t)b | ((uint32_t)(4 + b) << 4);
+  return __byte_perm(__byte_perm(h0, h1, sel), __byte_perm(h2, h3, sel), 0x5410);
+}
+
 // Unpack + split.  Output planes[t][(q, R)][C] want C-contiguous 128-byte lines, the input wants
-// q-contiguous runs, so: lane <-> q (32 consecutive q, 256-byte loads of one packed row), warp <->
-// one output row R, and the warp walks a whole 128-column block of that row in four 32-column
-// chunks -- every output line is completed by one thread within a few hundred cycles and leaves
-// L2 as a full line.  Blocks are ordered [128 x 128 super-tile pair (A >= B)][q chunk][sub]:
-// sub 0..15 = the 16 row groups of the (A, B) block (rows in A, columns in B), sub 16..31 = the
-// mirrored (B, A) block (rows in B, columns in A).  Both read the same 128 x 128 packed rows of
-// this q chunk (4 MB) back to back, so the second read is an L2 hit.
+// q-contiguous runs.  A warp owns one output row R and 8 consecutive q; lane = (qi, cg): q = q8 + qi,
+// columns cg*32 .. cg*32+31 of a 128-column block.  One load instruction reads 64-byte runs of
+// four packed rows; one store instruction writes pieces of only 8 output lines (a fully divergent
+// store costs 32 tag cycles in the LSU, which made the pass store-issue bound), and the four lanes
+// of a q complete its 128-byte line together.  A block = 2 rows x 32 q.  Blocks are ordered
+// [128 x 128 super-tile pair (A >= B)][q chunk][sub]: sub 0..63 = row pairs of the (A, B) block
+// (rows in A, columns in B), sub 64..127 = the mirrored (B, A) block; both read the same 128 x 128
+// packed rows of this q chunk (4 MB) back to back, so the second read is an L2 hit.
 template <int S>
 __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __restrict__ Bp, int nao, int naux,
                                                               int q0, int q1, const uint32_t* __restrict__ emax,
                                                               int32_t* __restrict__ e5, int8_t* __restrict__ planes,
                                                               long long pitch, long long plane_stride,
-                                                              int* __restrict__ status) {
+                                                              int* __restrict__ status, int dbg) {
   int A, B;
   bool lower;
-  const int sub = blockIdx.x & 31;
-  if (!tile_of_block(blockIdx.y, sub >> 4, A, B, lower)) return;  // (A, B) = (row block, column block)
+  const int sub = blockIdx.x & 127;
+  if (!tile_of_block(blockIdx.y, sub >> 6, A, B, lower)) return;  // (A, B) = (row block, column block)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int R = A * 128 + (sub & 15) * 8 + warp;
-  const int q = q0 + (blockIdx.x >> 5) * 32 + lane;
-  if (R >= nao || q >= q1) return;
+  const int R = A * 128 + (sub & 63) * 2 + (warp >> 2);
+  const int q = q0 + (blockIdx.x >> 7) * 32 + (warp & 3) * 8 + (lane >> 2);
+  const int C0 = B * 128 + (lane & 3) * 32;
+  if (R >= nao || q >= q1 || C0 >= pitch) return;
   const uint32_t hm = emax[(long long)R * naux + q];
   const int e = scale_index_from_hi(hm);
   const long long orow = (long long)(q - q0) * nao + R;
-  if (lower && B == 0) {
+  if (lower && C0 == 0) {
     e5[orow] = e;
     const int stt = status_from_hi(hm);
     if (stt) atomicOr(status, stt);
   }
   const double scale = pow2_double(63 - e);
   const double* bq = Bp + q;
-  for (int chunk = 0; chunk < 4; ++chunk) {
-    const int C0 = B * 128 + chunk * 32;
-    if (C0 >= pitch) break;
-    uint32_t w[S][8];
+  uint32_t w[S][8];
+  PackedRowWalker wk(R, C0);
+  // all loads of a half are issued before the first conversion (16 requests in flight per thread)
 #pragma unroll
-    for (int t = 0; t < S; ++t)
+  for (int half = 0; half < 2; ++half) {
+    double x[16];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) w[t][j] = 0;
-    PackedRowWalker wk(R, C0);
-    // all loads of a half chunk are issued before the first conversion (16 requests in flight)
+    for (int cc = 0; cc < 16; ++cc, wk.next())
+      x[cc] = (C0 + half * 16 + cc < nao && !(dbg & 2)) ? __ldg(bq + wk.p * naux) : 0.0;
 #pragma unroll
-    for (int half = 0; half < 2; ++half) {
-      double x[16];
+    for (int g4 = 0; g4 < 4; ++g4) {
+      uint32_t hi[4], lo[4];
 #pragma unroll
-      for (int cc = 0; cc < 16; ++cc, wk.next())
-        x[cc] = (C0 + half * 16 + cc < nao) ? __ldg(bq + wk.p * naux) : 0.0;
-#pragma unroll
-      for (int cc = 0; cc < 16; ++cc) {
-        const uint64_t dg = balanced_digits(x[cc], scale);
-        const int c32 = half * 16 + cc;
-#pragma unroll
-        for (int t = 0; t < S; ++t) w[t][c32 >> 2] |= digit_byte(dg, t) << (8 * (c32 & 3));
+      for (int j = 0; j < 4; ++j) {
+        const uint64_t dg = balanced_digits(x[4 * g4 + j], scale);
+        hi[j] = (uint32_t)(dg >> 32);
+        lo[j] = (uint32_t)dg;
       }
-    }
 #pragma unroll
-    for (int t = 0; t < S; ++t) {
-      uint4* dst = reinterpret_cast<uint4*>(planes + t * plane_stride + orow * pitch + C0);
-      dst[0] = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
-      dst[1] = make_uint4(w[t][4], w[t][5], w[t][6], w[t][7]);
+      for (int t = 0; t < S; ++t)
+        w[t][half * 4 + g4] = (t < 4) ? pack4_digit(hi[0], hi[1], hi[2], hi[3], 3 - t)
+                                      : pack4_digit(lo[0], lo[1], lo[2], lo[3], 7 - t);
     }
+  }
+#pragma unroll
+  for (int t = 0; t < S; ++t) {
+    uint4* dst = reinterpret_cast<uint4*>(planes + t * plane_stride + orow * pitch + C0);
+    if ((dbg & 1) && w[t][0] != 0x12345678u) continue;
+    dst[0] = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+    dst[1] = make_uint4(w[t][4], w[t][5], w[t][6], w[t][7]);
   }
 }
 
@@ -271,6 +280,9 @@ __global__ void __launch_bounds__(256) jk_j_unpack_kernel(const double* __restri
 }
 
 // ---------------------------------------------------------------------------
+static int g_jk_dbg = 0;
+void set_jk_debug_flags(int flags) { g_jk_dbg = flags; }
+
 static unsigned tile_pairs(int nao) {
   const unsigned T = (unsigned)((nao + 31) / 32);
   return T * (T + 1) / 2;
@@ -307,9 +319,9 @@ cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, 
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
                                    int* status, cudaStream_t st) {
   const unsigned T128 = (unsigned)((nao + 127) / 128);
-  dim3 grid(32u * (unsigned)((q1 - q0 + 31) / 32), T128 * (T128 + 1) / 2);
+  dim3 grid(128u * (unsigned)((q1 - q0 + 31) / 32), T128 * (T128 + 1) / 2);
   DFE_DISPATCH_S(s, (jk_unpack_split_kernel<SS><<<grid, 256, 0, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5,
-                                                                      pitch, plane_stride, status)));
+                                                                      pitch, plane_stride, status, g_jk_dbg)));
   count_launch();
   return cudaGetLastError();
 }

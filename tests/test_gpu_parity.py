@@ -294,3 +294,76 @@ def test_jk_naux_1_rank_one(dfe, gpu_ws):
     assert ng == 1
     assert np.allclose(J, np.sum(Bm * D) * Bm, rtol=1e-12, atol=1e-14 * np.abs(Bm).max())
     assert O.rel_frobenius(K, (Bm @ Cocc) @ (Bm @ Cocc).T) <= 1e-12
+
+
+def test_jk_medium_config2(dfe, gpu_ws):
+    """BASELINE.json config 2 (nao 500, naux 1700, nocc 50): several M tiles per q, four 512-q blocks,
+    full plain-FP64 oracle for J and K, oracle emulation for sampled q (bit-exact X)."""
+    cfg = G.CONFIGS["medium"]
+    Bp, Cocc, D = G.make_df_inputs(cfg)
+    J_ref, K_ref = O.df_jk_plain(Bp, cfg.nao, Cocc, D)
+    for tol in (1e-6, 1e-10):
+        s = dfe.df_slices_for_tol(tol)
+        J, K, X, e6, ng = run_jk(dfe, Bp, cfg.nao, cfg.naux, Cocc, cfg.nocc, D, s)
+        assert ng == len(O.q_groups(cfg.naux, cfg.nocc, s))
+        assert O.rel_frobenius(J, J_ref) <= 1e-12
+        assert O.rel_frobenius(K, K_ref) <= tol
+        assert np.array_equal(K, K.T) and np.array_equal(J, J.T)
+        for q in (0, 511, 512, 1699):
+            Xq = O.emul_x_group(Bp, cfg.nao, Cocc, s, q, q + 1)[0]
+            assert np.array_equal(X[:, q, :cfg.nocc], Xq), f"q={q}"
+    assert dfe.df_last_status() == 0
+
+
+def test_jk_large_config3_sampled(dfe, gpu_ws):
+    """Full size of the benchmark (config 3: nao 1200, naux 4000, nocc 150, packed B 23 GB generated on
+    the device), in bench.py's launch configuration (all 4000 q in one super-block).  The oracle
+    computes sampled outputs one by one from the same bytes: rho (all of it, streamed back in
+    chunks), sampled J entries, sampled K entries; plus the invariants that hold at any size."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 75 << 30:
+        pytest.skip("needs ~70 GB of free device memory")
+    cfg = G.CONFIGS["large"]
+    nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc
+    tol = 2.0 ** -23
+    s = dfe.df_slices_for_tol(tol)
+    B = G.make_B_packed_torch(nao, naux, cfg.seed, device=DEV)
+    Cocc = G.make_C_occ(nao, nocc, cfg.seed)
+    D = G.make_density(Cocc)
+    big = dfe.Workspace(dfe.df_jk_workspace_bytes_blocks(nao, naux, nocc, s, 8))
+    try:
+        J = torch.empty((nao, nao), dtype=torch.float64, device=DEV)
+        K = torch.empty_like(J)
+        dfe.df_jk_build(B, nao, naux, dev(Cocc), nocc, dev(D), tol, J, K)
+        torch.cuda.synchronize()
+        assert dfe.df_last_status() == 0
+    finally:
+        big.close()
+        dfe.df_set_workspace(gpu_ws.view)
+    Jh, Kh = J.cpu().numpy(), K.cpu().numpy()
+    assert np.array_equal(Jh, Jh.T) and np.array_equal(Kh, Kh.T)
+    # rho by the oracle's definition, streamed: rho = (w * d) @ B_packed
+    il, jl = np.tril_indices(nao)
+    wd = np.where(il == jl, 1.0, 2.0) * 0.5 * (D[il, jl] + D[jl, il])
+    rho = np.zeros(naux)
+    step = 40000
+    for p0 in range(0, il.size, step):
+        rho += wd[p0:p0 + step] @ B[p0:p0 + step].cpu().numpy()
+    assert abs(np.sum(D * Jh) - rho @ rho) <= 1e-11 * (rho @ rho)  # Tr(D J) = |rho|^2
+    rng = np.random.default_rng(0)
+    for (i, j) in [(0, 0), (1199, 1199), (700, 3), (1199, 0)] + [tuple(sorted(rng.integers(0, nao, 2))[::-1]) for _ in range(4)]:
+        p = i * (i + 1) // 2 + j
+        Jp = float(B[p].cpu().numpy() @ rho)
+        assert abs(Jh[i, j] - Jp) <= 1e-11 * np.abs(Jh).max(), (i, j)
+    # sampled K entries: X_i[q, a] = sum_j B^q_ij C_ja from the packed rows of i
+    def x_rows(i):
+        idx = torch.tensor([max(i, j) * (max(i, j) + 1) // 2 + min(i, j) for j in range(nao)], device=DEV)
+        Bi = B.index_select(0, idx).cpu().numpy()  # (nao j, naux q)
+        return Bi.T @ Cocc                          # (naux, nocc)
+    rows = {i: x_rows(i) for i in (0, 5, 700, 1199)}
+    for i in rows:
+        for j in rows:
+            kij = float(np.sum(rows[i] * rows[j]))
+            scale = np.sqrt(np.sum(rows[i] ** 2) * np.sum(rows[j] ** 2))
+            assert abs(Kh[i, j] - kij) <= tol * scale, (i, j, Kh[i, j], kij)
+    assert np.sum(D * Kh) >= 0.0  # Tr(D K) = 2 |C^T X|^2 (DESIGN.md R8)
