@@ -146,7 +146,7 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB,
                          int bk, int32_t* P, void* stream);
 
 /* df_jk_build_slices that also exports GEMM(5)'s FP64 output
- * X[i][q][a_pad] (a_pad = 16*ceil(nocc/16), padded columns are zero) and the
+ * X[q][i][a_pad] (a_pad = 16*ceil(nocc/16), padded columns are zero) and the
  * GEMM(6) scale indices e6[g][i] of every q-group g (R5).  X_out /
  * e6_out may be NULL.  *ngroups_out (host) receives the number of groups. */
 int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
@@ -157,6 +157,11 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
 /* Timing experiments on the GEMM kernel (results are then garbage): bit 0 = issue no
  * MMAs (operand feed only), bit 1 = issue no TMA loads (MMA issue only).  0 = normal. */
 int df_debug_set_gemm_flags(int flags);
+
+/* Cycle counters CTA 0 of the last GEMM(5) launch left in the workspace (timing experiments):
+ * {epilogue wait, epilogue work, MMA-warp wait for operands, MMA-warp wait for TMEM, MMA-warp total}.
+ * Synchronises the device. */
+int df_debug_read_clocks(int64_t* out8);
 
 /* Number of GPU kernels this library has launched in this process. */
 int64_t df_launch_count(void);

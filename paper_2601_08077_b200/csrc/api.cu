@@ -21,6 +21,7 @@ static int64_t g_ws_bytes = 0;
 static int g_mode = DF_MODE_GUARDED;
 static int g_device_ok = -1;
 static int g_g5_split_n = 1;
+static int g_g5_cluster = 1;
 
 // ---- optional per-kernel-class CUDA-event timing (df_profile_*; bench.py's roofline) ----
 enum ProfClass { kPSplit = 0, kPPassA, kPJGemv, kPUnpack, kPGemm5, kPSplitX, kPGemm6, kPReduce, kPGemm, kPNum };
@@ -333,27 +334,29 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) g5.n_tile = w.a_pad / 2;
     g5.acc_stride = (g5.n_tile % 32) ? g5.n_tile : 0;
     g5.x_cols = w.a_pad;
+    g5.cluster_n = (g_g5_cluster && g5.n_tile * 2 == w.a_pad) ? 2 : 1;
     g5.nz = 1;
     g5.eA = w.e5;
     g5.eB = w.eC;
     g5.mode = kEpiX;
     g5.C = w.X;
     g5.nao = (int)nao;
-    g5.ldx = ncol;
+    g5.ldx = w.a_pad;
     g5.qgroup = w.qgroup;
     g5.xmax = w.xmax;
+    g5.dbg_clk = (long long*)(w.status + 16);  // 8 counters inside the 256-byte status block
     {
       ProfScope ps(kPGemm5, st);
       DFE_CK(launch_gemm_i8(g5, st));
     }
     if (X_out)
-      DFE_CK(cudaMemcpy2DAsync(X_out + qs0 * w.a_pad, sizeof(double) * naux * w.a_pad, w.X, sizeof(double) * ncol,
-                               sizeof(double) * ncol, nao, cudaMemcpyDeviceToDevice, st));
+      DFE_CK(cudaMemcpyAsync(X_out + qs0 * nao * w.a_pad, w.X, sizeof(double) * nq * nao * w.a_pad,
+                             cudaMemcpyDeviceToDevice, st));
 
     // X -> planes6 with one scale per (i, group)
     {
       ProfScope ps(kPSplitX, st);
-      DFE_CK(launch_jk_split_x(w.X, (int)nao, ncol, ncol, s, ng, w.gcol, w.xmax, w.e6, w.p6, pitch6,
+      DFE_CK(launch_jk_split_x(w.X, (int)nao, nq, w.a_pad, s, ng, w.qgroup, w.xmax, w.e6, w.p6, pitch6,
                                (int64_t)nao * pitch6, w.status, st));
     }
     if (e6_out)
@@ -558,7 +561,16 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t 
 int df_debug_set_gemm_flags(int flags) {
   set_gemm_debug_flags(flags);
   g_g5_split_n = (flags & 4) ? 0 : 1;
-  set_jk_debug_flags((flags >> 4) & 3);  // bits 4, 5: unpack kernel without stores / without loads  // bit 2: GEMM(5) keeps one N tile (multi-pass read-modify-write)
+  g_g5_cluster = (flags & 64) ? 0 : 1;  // bit 6: GEMM(5) without the cluster-pair multicast
+  set_jk_debug_flags((flags >> 4) & 3);
+  set_peak_tiles((flags >> 16) & 15);  // bits 16,17: MMA probe walks 1..4 operand tiles; bits 18,19: swizzle 32/64/128  // bits 4, 5: unpack kernel without stores / without loads  // bit 2: GEMM(5) keeps one N tile (multi-pass read-modify-write)
+  return DF_OK;
+}
+
+int df_debug_read_clocks(int64_t* out8) {
+  if (!out8) return DF_ERR_NULL;
+  if (!g_ws) return DF_ERR_WORKSPACE;
+  if (cudaMemcpy(out8, (char*)g_ws + 64, 8 * sizeof(int64_t), cudaMemcpyDeviceToHost) != cudaSuccess) return DF_ERR_CUDA;
   return DF_OK;
 }
 

@@ -23,14 +23,16 @@
 namespace dfe {
 
 constexpr int kMaxStages = 8;
-constexpr int kGemmThreads = 192;
-constexpr int kSmemLimit = 232448 - 19456;  // 227 KB minus the static shared memory (barriers, epilogue staging)
+constexpr int kGemmThreads = 320;  // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue (two per TMEM lane quarter)
+constexpr int kSmemLimit = 232448 - 21504;  // 227 KB minus the static shared memory (barriers, epilogue staging)
 
 struct GemmKernelParams {
   CUtensorMap mapA;
   CUtensorMap mapB;
+  CUtensorMap mapA2;  // A planes with a 64-row box (cluster pair: each CTA loads and multicasts half a tile)
   int s, n_tile, acc_stride, weights_per_pass;
-  int tiles_m, tiles_n, group_m;
+  int tiles_m, tiles_n, group_m, tiles_per_z;
+  long long total_work;
   int num_stages;
   uint32_t stage_stride;
   long long a_rows, b_rows;
@@ -54,6 +56,7 @@ struct GemmKernelParams {
   // [pass_start[ps], pass_start[ps+1])
   uint2 pairs[kMaxSlices * (kMaxSlices + 1) / 2];
   int pass_start[kMaxSlices + 1];
+  long long* dbg_clk;  // optional: cycles of CTA 0 {epilogue wait, epilogue work, MMA-warp wait, MMA-warp issue, producer wait}
   int dbg_flags;  // bit 0: no MMAs (operand feed only); bit 1: no TMA loads (MMA issue only)
 };
 
@@ -63,23 +66,55 @@ __device__ __forceinline__ void pass_weights(int s, int W, int ps, int& w_hi, in
   w_lo = max(2, w_hi - W + 1);
 }
 
-template <int BK>
-__global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_constant__ GemmKernelParams p) {
-  // ---- tile coordinates (grouped rasterisation: bands of group_m tile rows) ----
-  int tm, tn;
-  {
-    const int lin = blockIdx.x;
+// One unit of work of the persistent kernel: an output tile of one z item.
+struct WorkItem {
+  int tm, tn, z, zk0, zk1, chunk_lo, chunk_hi;
+};
+
+// Work index -> tile.  z is the slowest index; inside a z item tiles are rasterised in bands of
+// group_m tile rows (operand reuse in L2), or -- lower_only -- over the pairs tm >= tn.
+__device__ __forceinline__ WorkItem decode_work(const GemmKernelParams& p, long long wi) {
+  WorkItem w;
+  w.z = (int)(wi / p.tiles_per_z);
+  const int lin = (int)(wi - (long long)w.z * p.tiles_per_z);
+  if (p.lower_only) {
+    int a = (int)((sqrtf(8.0f * (float)lin + 1.0f) - 1.0f) * 0.5f);
+    while ((a + 1) * (a + 2) / 2 <= lin) ++a;
+    while (a * (a + 1) / 2 > lin) --a;
+    w.tm = a;
+    w.tn = lin - a * (a + 1) / 2;
+  } else {
     const int per_band = p.group_m * p.tiles_n;
     const int band = lin / per_band;
     const int first_m = band * p.group_m;
     const int gm = min(p.group_m, p.tiles_m - first_m);
     const int r = lin - band * per_band;
-    tm = first_m + r % gm;
-    tn = r / gm;
+    w.tm = first_m + r % gm;
+    w.tn = r / gm;
   }
-  if (p.lower_only && tn > tm) return;  // block-uniform, before any allocation
-  const int z = blockIdx.z;
+  w.zk0 = p.zk ? p.zk[w.z] : 0;
+  w.zk1 = p.zk ? p.zk[w.z + 1] : p.k;
+  w.chunk_lo = 0;
+  w.chunk_hi = max(1, (w.zk1 - w.zk0 + p.kflush - 1) / p.kflush);
+  if (p.mode == kEpiInt32) {
+    w.chunk_lo = p.dbg_chunk;
+    w.chunk_hi = p.dbg_chunk + 1;
+  }
+  return w;
+}
 
+#define DFE_WORK_LOOP                                                                  \
+  for (long long wi = (CL == 1) ? (long long)blockIdx.x : (long long)(blockIdx.x & ~1u) + crank; wi < p.total_work;  \
+       wi += gridDim.x) {                                                              \
+    const WorkItem wk = decode_work(p, wi);                                            \
+    const int tm = wk.tm, tn = wk.tn, z = wk.z, zk0 = wk.zk0, zk1 = wk.zk1;            \
+    const int chunk_lo = wk.chunk_lo, chunk_hi = wk.chunk_hi;                          \
+    (void)tm; (void)tn; (void)z; (void)zk0; (void)zk1;
+
+// Persistent: grid = min(work items, SMs); every role walks the same work sequence, the pipeline
+// counters run on across tiles, so the producer prefetches the next tile during the epilogue.
+template <int BK, int CL>
+__global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_constant__ GemmKernelParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t full_bar[kMaxStages];
@@ -87,7 +122,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   __shared__ __align__(8) uint64_t tmem_full_bar;
   __shared__ __align__(8) uint64_t tmem_empty_bar;
   __shared__ uint32_t tmem_slot;
-  __shared__ __align__(16) double epi_stage[4][32][18];  // per epilogue warp: 32 rows x 16 cols, 144 B pitch
+  __shared__ __align__(16) double epi_stage[8][32][10];  // per epilogue warp: 32 rows x 8 cols, 80 B pitch
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -95,31 +130,26 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   const int W = p.weights_per_pass;
   const int npass = (s + W - 1) / W;
   const int S = p.num_stages;
-
-  // contraction range of this z item and its flush chunks
-  const int zk0 = p.zk ? p.zk[z] : 0;
-  const int zk1 = p.zk ? p.zk[z + 1] : p.k;
-  int chunk_lo = 0;
-  int chunk_hi = max(1, (zk1 - zk0 + p.kflush - 1) / p.kflush);
-  if (p.mode == kEpiInt32) {
-    chunk_lo = p.dbg_chunk;
-    chunk_hi = p.dbg_chunk + 1;
-  }
+  // CL == 2: a cluster of two CTAs owns the two N tiles of one M tile (work items 2c, 2c+1); each
+  // loads half of every A plane tile and multicasts it to both, so the A operand crosses L2 once.
+  const uint32_t crank = (CL == 2) ? cluster_ctarank() : 0u;
+  (void)crank;
 
   if (warp == 0 && lane == 0) {
     prefetch_tensormap(&p.mapA);
     prefetch_tensormap(&p.mapB);
     for (int i = 0; i < S; ++i) {
       mbar_init(&full_bar[i], 1);
-      mbar_init(&empty_bar[i], 1);
+      mbar_init(&empty_bar[i], CL);
     }
     mbar_init(&tmem_full_bar, 1);
-    mbar_init(&tmem_empty_bar, 128);
+    mbar_init(&tmem_empty_bar, kGemmThreads - 64);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(&tmem_slot, 512);
   tc_fence_before();
   __syncthreads();
+  if (CL == 2) cluster_sync_all();  // the peer's barriers are initialised before anything arrives on them
   tc_fence_after();
   const uint32_t tmem_base = tmem_slot;
 
@@ -131,6 +161,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     // ================= TMA producer =================
     if (lane == 0) {
       uint32_t it = 0;
+      DFE_WORK_LOOP
       for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
         const int kc0 = zk0 + ch * p.kflush;
         const int kc1 = min(zk1, kc0 + p.kflush);
@@ -151,13 +182,20 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             uint8_t* st = smem + (size_t)stage * p.stage_stride;
             mbar_expect_tx(&full_bar[stage], tx);
             const int kpos = kc0 + kb * BK;
-            for (int t = 0; t < P; ++t)
-              tma_load_3d(st + t * a_plane_bytes, &p.mapA, &full_bar[stage], kpos, tm * kTileM, t);
+            if (CL == 2) {
+              for (int t = 0; t < P; ++t)
+                tma_load_3d_mcast(st + t * a_plane_bytes + crank * (64 * BK), &p.mapA2, &full_bar[stage], kpos,
+                                  tm * kTileM + (int)crank * 64, t, (uint16_t)3);
+            } else {
+              for (int t = 0; t < P; ++t)
+                tma_load_3d(st + t * a_plane_bytes, &p.mapA, &full_bar[stage], kpos, tm * kTileM, t);
+            }
             for (int u = 0; u < P; ++u)
               tma_load_3d(st + b_off + u * b_plane_bytes, &p.mapB, &full_bar[stage], kpos, tn * p.n_tile, u);
           }
         }
       }
+      }  // work loop
     }
   } else if (warp == 1) {
     // ================= MMA issuer =================
@@ -172,6 +210,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     const uint32_t smem_base16 = (smem_u32(smem) & 0x3FFFFu) >> 4;
     const uint32_t stage16 = p.stage_stride >> 4;
     uint32_t it = 0, iter = 0;
+    long long clk_mwait = 0, clk_tmem = 0;
+    const long long clk_m0 = clock64();
+    DFE_WORK_LOOP
     for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
       const int kc0 = zk0 + ch * p.kflush;
       const int kc1 = min(zk1, kc0 + p.kflush);
@@ -179,14 +220,18 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
       for (int ps = 0; ps < npass; ++ps, ++iter) {
         const int pr0 = p.pass_start[ps], pr1 = p.pass_start[ps + 1];
         if (iter > 0) {
+          const long long tt0 = clock64();
           mbar_wait(&tmem_empty_bar, (iter - 1) & 1u);
           tc_fence_after();
+          clk_tmem += clock64() - tt0;
         }
         for (int kb = 0; kb < nkb; ++kb, ++it) {
           const uint32_t stage = it % S;
           const uint32_t ph = (it / S) & 1u;
+          const long long tw0 = clock64();
           mbar_wait(&full_bar[stage], ph);
           tc_fence_after();
+          clk_mwait += clock64() - tw0;
           if (p.dbg_flags & 1) {
             if (lane == 0) mbar_arrive(&empty_bar[stage]);
             continue;
@@ -206,7 +251,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
                 mma_i8_ss(tmem_base + (e.y & 0xFFFFu), adesc, bdesc, idesc, later | (e.y >> 16));
               }
             }
-            mma_commit(&empty_bar[stage]);  // frees the smem stage once these MMAs have read it
+            // frees the smem stage once these MMAs have read it (in both CTAs of a pair: the peer
+            // multicasts into this stage too)
+            if (CL == 2) mma_commit_mcast(&empty_bar[stage], (uint16_t)3);
+            else mma_commit(&empty_bar[stage]);
           }
           __syncwarp();
         }
@@ -214,9 +262,18 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         __syncwarp();
       }
     }
+    }  // work loop
+    if (p.dbg_clk && blockIdx.x == 0 && lane == 0) {
+      p.dbg_clk[2] = clk_mwait;
+      p.dbg_clk[3] = clk_tmem;
+      p.dbg_clk[4] = clock64() - clk_m0;
+    }
   } else {
     // ================= epilogue: TMEM -> FP64 recombination -> global =================
     const int quarter = warp & 3;
+    uint32_t iter = 0;
+    long long clk_wait = 0, clk_work = 0;
+    DFE_WORK_LOOP
     const int row_local = quarter * 32 + lane;
     const long long row = (long long)tm * kTileM + row_local;
     const bool row_ok = row < p.a_rows;
@@ -228,31 +285,30 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     if (p.mode == kEpiC) {
       out = p.C + z * p.c_stride + row * p.ldc;
     } else if (p.mode == kEpiX) {
-      const long long q = row / p.nao;
-      const long long i = row - q * p.nao;
-      out = p.C + i * p.ldx + q * p.x_cols;  // indexed by the global column
+      out = p.C + row * p.ldx;  // X[(q, i)][a_pad]: the tile is one contiguous block
     }
-    // coalesced phase: lane moves columns cpair, cpair+1 of rows (lane >> 3) + 4 j, j = 0..7
-    const int cpair = (lane & 7) * 2;
-    double(*stg)[18] = epi_stage[quarter];
-    double* srow[8];
+    // two epilogue warps per lane quarter: warps 2..5 take the even 16-column blocks, 6..9 the odd
+    const int chalf = (warp - 2) >> 2;
+    // coalesced phase: lane moves columns cpair, cpair+1 (of an 8-column half block) of rows
+    // (lane >> 2) + 8 j, j = 0..3: one store instruction covers 8 rows x 64 bytes
+    const int cpair = (lane & 3) * 2;
+    double(*stg)[10] = epi_stage[warp - 2];
+    double* srow[4];
     const long long ld_out = (p.mode == kEpiX) ? p.ldx : p.ldc;
     const bool vec_ok = p.mode != kEpiInt32 && ((ld_out | p.c_stride | (long long)col0) & 1) == 0 &&
                         ((uintptr_t)p.C & 15) == 0;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      const long long rr = (long long)tm * kTileM + quarter * 32 + (lane >> 3) + 4 * j;
+    for (int j = 0; j < 4; ++j) {
+      const long long rr = (long long)tm * kTileM + quarter * 32 + (lane >> 2) + 8 * j;
       srow[j] = nullptr;
       if (rr < p.a_rows) {
         if (p.mode == kEpiC) {
           srow[j] = p.C + z * p.c_stride + rr * p.ldc;
         } else if (p.mode == kEpiX) {
-          const long long q = rr / p.nao;
-          srow[j] = p.C + (rr - q * p.nao) * p.ldx + q * p.x_cols;
+          srow[j] = p.C + rr * p.ldx;
         }
       }
     }
-    uint32_t iter = 0;
     uint32_t hi_max = 0;
     for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
       for (int ps = 0; ps < npass; ++ps, ++iter) {
@@ -260,9 +316,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         pass_weights(s, W, ps, w_hi, w_lo);
         const bool first = (ch == chunk_lo) && (ps == 0);
         const bool last = (ch == chunk_hi - 1) && (ps == npass - 1);
+        const long long t0 = clock64();
         mbar_wait(&tmem_full_bar, iter & 1u);
         tc_fence_after();
-        for (int c = 0; c < p.n_tile; c += 16) {
+        const long long t1 = clock64();
+        clk_wait += t1 - t0;
+        for (int c = chalf * 16; c < p.n_tile; c += 32) {
           uint32_t v[16];
           if (p.mode == kEpiInt32) {
             for (int w = w_hi; w >= w_lo; --w) {
@@ -286,26 +345,29 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             eBv[j] = (row_ok && col < p.b_rows) ? p.eB[z * p.eb_stride + col] : 0;
             acc[j] = 0.0;
           }
-          const long long colv = col0 + c + cpair;  // first of the two columns this lane moves
           if (!first) {
-            // running sum of the earlier passes/chunks: coalesced 16-byte loads (8 lanes cover one
-            // row's 128 bytes), transposed through shared memory to "lane = row"
+            // running sum of the earlier passes/chunks: coalesced 16-byte loads (4 lanes cover 64
+            // bytes of a row), transposed through shared memory to "lane = row"
             if (vec_ok) {
 #pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                double2 v = make_double2(0.0, 0.0);
-                if (srow[j] && colv + 1 < p.b_rows) v = *reinterpret_cast<const double2*>(srow[j] + colv);
-                else if (srow[j] && colv < p.b_rows) v.x = srow[j][colv];
-                *reinterpret_cast<double2*>(&stg[(lane >> 3) + 4 * j][cpair]) = v;
-              }
-              __syncwarp();
+              for (int h = 0; h < 2; ++h) {
+                const long long colv = col0 + c + 8 * h + cpair;
 #pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                const double2 v = *reinterpret_cast<const double2*>(&stg[lane][2 * j]);
-                acc[2 * j] = v.x;
-                acc[2 * j + 1] = v.y;
+                for (int j = 0; j < 4; ++j) {
+                  double2 v2 = make_double2(0.0, 0.0);
+                  if (srow[j] && colv + 1 < p.b_rows) v2 = *reinterpret_cast<const double2*>(srow[j] + colv);
+                  else if (srow[j] && colv < p.b_rows) v2.x = srow[j][colv];
+                  *reinterpret_cast<double2*>(&stg[(lane >> 2) + 8 * j][cpair]) = v2;
+                }
+                __syncwarp();
+#pragma unroll
+                for (int k2 = 0; k2 < 4; ++k2) {
+                  const double2 v2 = *reinterpret_cast<const double2*>(&stg[lane][2 * k2]);
+                  acc[8 * h + 2 * k2] = v2.x;
+                  acc[8 * h + 2 * k2 + 1] = v2.y;
+                }
+                __syncwarp();
               }
-              __syncwarp();
             } else {
 #pragma unroll
               for (int j = 0; j < 16; ++j) {
@@ -329,16 +391,20 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
           }
           if (vec_ok) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
-              *reinterpret_cast<double2*>(&stg[lane][2 * j]) = make_double2(acc[2 * j], acc[2 * j + 1]);
-            __syncwarp();
+            for (int h = 0; h < 2; ++h) {
+              const long long colv = col0 + c + 8 * h + cpair;
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              const double2 v = *reinterpret_cast<const double2*>(&stg[(lane >> 3) + 4 * j][cpair]);
-              if (srow[j] && colv + 1 < p.b_rows) *reinterpret_cast<double2*>(srow[j] + colv) = v;
-              else if (srow[j] && colv < p.b_rows) srow[j][colv] = v.x;
+              for (int k2 = 0; k2 < 4; ++k2)
+                *reinterpret_cast<double2*>(&stg[lane][2 * k2]) = make_double2(acc[8 * h + 2 * k2], acc[8 * h + 2 * k2 + 1]);
+              __syncwarp();
+#pragma unroll
+              for (int j = 0; j < 4; ++j) {
+                const double2 v2 = *reinterpret_cast<const double2*>(&stg[(lane >> 2) + 8 * j][cpair]);
+                if (srow[j] && colv + 1 < p.b_rows) *reinterpret_cast<double2*>(srow[j] + colv) = v2;
+                else if (srow[j] && colv < p.b_rows) srow[j][colv] = v2.x;
+              }
+              __syncwarp();
             }
-            __syncwarp();
           } else {
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
@@ -349,6 +415,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         }
         tc_fence_before();
         mbar_arrive(&tmem_empty_bar);
+        clk_work += clock64() - t1;
       }
     }
     if (p.mode == kEpiX && row_ok) {
@@ -356,10 +423,16 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
       const long long i = row - q * p.nao;
       atomicMax(&p.xmax[(long long)p.qgroup[q] * p.nao + i], hi_max);
     }
+    }  // work loop
+    if (p.dbg_clk && blockIdx.x == 0 && warp == 2 && lane == 0) {
+      p.dbg_clk[0] = clk_wait;
+      p.dbg_clk[1] = clk_work;
+    }
   }
 
   tc_fence_before();
   __syncthreads();
+  if (CL == 2) cluster_sync_all();  // no CTA leaves while its peer may still write to it
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc(tmem_base, 512);
@@ -370,14 +443,22 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
 // tcgen05.mma.kind::i8 issue-rate probe: operands resident in shared memory, no loads.
 // MEASURED_PEAKS.json has no INT8 figure; this gives the roofline denominator.
 // ---------------------------------------------------------------------------
-__global__ void __launch_bounds__(128, 1) mma_peak_kernel(int n_mma, int iters) {
+static int g_peak_tiles = 1, g_peak_swz = 32;
+void set_peak_tiles(int n) {
+  g_peak_tiles = (n & 3) + 1;                                   // 1..4 distinct operand tiles
+  g_peak_swz = ((n >> 2) & 3) == 1 ? 64 : ((n >> 2) & 3) == 2 ? 128 : 32;  // swizzle span of the tiles
+}
+
+__global__ void __launch_bounds__(128, 1) mma_peak_kernel(int n_mma, int iters, int ntiles, int swz) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t done_bar;
   __shared__ uint32_t tmem_slot;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  // A: 128 rows x 32 B (SW32 tile, 4 KB), B: n_mma rows x 32 B, zero-filled
-  for (int i = threadIdx.x; i < (128 + 256) * 32 / 4; i += blockDim.x) ((uint32_t*)smem)[i] = 0;
+  // ntiles A tiles of 128 rows x 32 B (SW32, 4 KB each) and ntiles B tiles of 256 rows x 32 B,
+  // zero-filled; ntiles > 1 walks different tiles so that no operand can be reused from the
+  // previous MMA (shared-memory operand bandwidth shows).
+  for (int i = threadIdx.x; i < ntiles * (128 + 256) * swz / 4; i += blockDim.x) ((uint32_t*)smem)[i] = 0;
   if (threadIdx.x == 0) {
     mbar_init(&done_bar, 1);
     fence_barrier_init();
@@ -388,12 +469,24 @@ __global__ void __launch_bounds__(128, 1) mma_peak_kernel(int n_mma, int iters) 
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_slot;
-  if (warp == 0 && lane == 0) {
+  if (warp == 0) {
     const uint32_t idesc = make_idesc_i8(128, n_mma);
-    const uint64_t adesc = make_smem_desc(smem_u32(smem), 32);
-    const uint64_t bdesc = make_smem_desc(smem_u32(smem + 128 * 32), 32);
-    for (int i = 0; i < iters; ++i) mma_i8_ss(tmem_base + (uint32_t)((i & 1) * 256), adesc, bdesc, idesc, i > 1);
-    mma_commit(&done_bar);
+    const uint64_t proto = make_smem_desc(0, swz);
+    const uint32_t a_t16 = 128u * swz / 16u, b_t16 = 256u * swz / 16u, nk = swz / 32;
+    const uint32_t hi = (uint32_t)(proto >> 32), lo0 = (uint32_t)proto;
+    const uint32_t a16 = (smem_u32(smem) & 0x3FFFFu) >> 4, b16 = a16 + (uint32_t)ntiles * a_t16;
+    if (elect_one()) {
+      int ta = 0, tb = 0;
+      for (int i = 0; i < iters; ++i) {
+        const uint32_t kk2 = 2u * ((uint32_t)i % nk);  // K step inside the swizzle row, 16-byte units
+        const uint64_t adesc = ((uint64_t)hi << 32) | (lo0 | (a16 + (uint32_t)ta * a_t16 + kk2));
+        const uint64_t bdesc = ((uint64_t)hi << 32) | (lo0 | (b16 + (uint32_t)tb * b_t16 + kk2));
+        mma_i8_ss(tmem_base + (uint32_t)((i & 1) * 256), adesc, bdesc, idesc, i > 1);
+        if (++ta == ntiles) { ta = 0; if (++tb == ntiles) tb = 0; }
+      }
+      mma_commit(&done_bar);
+    }
+    __syncwarp();
     mbar_wait(&done_bar, 0);
   }
   tc_fence_before();
@@ -405,14 +498,17 @@ __global__ void __launch_bounds__(128, 1) mma_peak_kernel(int n_mma, int iters) 
 }
 
 cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStream_t st) {
-  cudaError_t err = cudaFuncSetAttribute(mma_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384);
+  const int ntiles = g_peak_tiles;
+  const int swz = g_peak_swz;
+  const int smem_bytes = ntiles * (128 + 256) * swz + 2048;
+  cudaError_t err = cudaFuncSetAttribute(mma_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
   if (err != cudaSuccess) return err;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0);
   cudaEventCreate(&e1);
-  mma_peak_kernel<<<grid, 128, 16384, st>>>(n_mma, 64);  // warm-up
+  mma_peak_kernel<<<grid, 128, smem_bytes, st>>>(n_mma, 64, ntiles, swz);  // warm-up
   cudaEventRecord(e0, st);
-  mma_peak_kernel<<<grid, 128, 16384, st>>>(n_mma, iters);
+  mma_peak_kernel<<<grid, 128, smem_bytes, st>>>(n_mma, iters, ntiles, swz);
   cudaEventRecord(e1, st);
   count_launch(2);
   err = cudaEventSynchronize(e1);
@@ -505,12 +601,22 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
     for (int ps = 0; ps < npass; ++ps) {
       p.pass_start[ps] = np;
       const int w_hi = s + 1 - ps * W, w_lo = (w_hi - W + 1) > 2 ? (w_hi - W + 1) : 2;
-      for (int w = w_hi; w >= w_lo; --w) {
-        const int t_lo = (w - s) > 1 ? (w - s) : 1, t_hi = (w - 1) < s ? (w - 1) : s;
-        for (int t = t_lo; t <= t_hi; ++t, ++np) {
+      // round-robin over the weights of the pass, so that consecutive MMAs target different TMEM
+      // accumulators (back-to-back MMAs into one accumulator wait on each other)
+      int next_t[kMaxSlices + 2];
+      for (int w = w_lo; w <= w_hi; ++w) next_t[w] = (w - s) > 1 ? (w - s) : 1;
+      for (bool any = true; any;) {
+        any = false;
+        for (int w = w_hi; w >= w_lo; --w) {
+          const int t_lo = (w - s) > 1 ? (w - s) : 1, t_hi = (w - 1) < s ? (w - 1) : s;
+          const int t = next_t[w];
+          if (t > t_hi) continue;
+          any = true;
+          next_t[w] = t + 1;
           const uint32_t ao = ((uint32_t)(t - 1) * a_plane) >> 4, bo = (b_off + (uint32_t)(w - t - 1) * b_plane) >> 4;
           p.pairs[np].x = ao | (bo << 16);
           p.pairs[np].y = (uint32_t)((w_hi - w) * p.acc_stride) | ((t > t_lo ? 1u : 0u) << 16);
+          ++np;
         }
       }
     }
@@ -541,20 +647,52 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.P = g.P;
   p.dbg_chunk = g.dbg_chunk;
   p.dbg_flags = g_gemm_dbg_flags;
+  p.dbg_clk = g.dbg_clk;
 
+  p.tiles_per_z = g.lower_only ? p.tiles_m * (p.tiles_m + 1) / 2 : p.tiles_m * p.tiles_n;
+  p.total_work = (long long)p.tiles_per_z * g.nz;
+  static int num_sms = 0;
+  if (!num_sms) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+  }
   const size_t smem = (size_t)p.num_stages * p.stage_stride + 1024;
-  dim3 grid((unsigned)((int64_t)p.tiles_m * p.tiles_n), 1, (unsigned)g.nz);
+  // cluster pair: the two N tiles of an M tile share the A operand through TMA multicast
+  const int cl = (g.cluster_n == 2 && p.tiles_n == 2 && !g.lower_only && g_gemm_dbg_flags == 0 && num_sms >= 2) ? 2 : 1;
+  if (cl == 2) {
+    p.group_m = 1;  // work items 2c, 2c+1 = (tm = c, tn = 0 / 1)
+    if (!make_plane_map(&p.mapA2, g.A, g.k, g.a_rows, s, g.a_pitch, g.a_plane_stride, bk, 64)) return cudaErrorInvalidValue;
+  }
+  // persistent when tiles are short (the per-CTA set-up of ~4 us would show); long-K tiles are left
+  // to the hardware scheduler, which balances them better than a static round-robin
+  const long long k_item = g.zk ? g.k / (g.nz > 0 ? g.nz : 1) : g.k;
+  const bool persistent = cl == 2 || k_item <= 8192;
+  long long nblocks = p.total_work;
+  if (persistent && nblocks > num_sms) nblocks = num_sms;
+  if (cl == 2) nblocks = (nblocks + 1) / 2 * 2;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)nblocks, 1, 1);
+  cfg.blockDim = dim3(kGemmThreads, 1, 1);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = cl;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
   cudaError_t err;
-#define DFE_LAUNCH(BKV)                                                                                 \
-  err = cudaFuncSetAttribute(gemm_i8_kernel<BKV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-  if (err != cudaSuccess) return err;                                                                   \
-  gemm_i8_kernel<BKV><<<grid, kGemmThreads, smem, st>>>(p);
-  if (bk == 128) {
-    DFE_LAUNCH(128)
-  } else if (bk == 64) {
-    DFE_LAUNCH(64)
+#define DFE_LAUNCH(BKV, CLV)                                                                                    \
+  err = cudaFuncSetAttribute(gemm_i8_kernel<BKV, CLV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+  if (err != cudaSuccess) return err;                                                                           \
+  err = cudaLaunchKernelEx(&cfg, gemm_i8_kernel<BKV, CLV>, p);                                                  \
+  if (err != cudaSuccess) return err;
+  if (cl == 2) {
+    if (bk == 128) { DFE_LAUNCH(128, 2) } else if (bk == 64) { DFE_LAUNCH(64, 2) } else { DFE_LAUNCH(32, 2) }
   } else {
-    DFE_LAUNCH(32)
+    if (bk == 128) { DFE_LAUNCH(128, 1) } else if (bk == 64) { DFE_LAUNCH(64, 1) } else { DFE_LAUNCH(32, 1) }
   }
 #undef DFE_LAUNCH
   count_launch();

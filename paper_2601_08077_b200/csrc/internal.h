@@ -46,12 +46,13 @@ struct GemmProblem {
   const int32_t* eA;  // scale indices, eA[z * ea_stride + row]
   const int32_t* eB;
   int64_t ea_stride, eb_stride;
+  int cluster_n;      // 2: CTA pairs over the two N tiles share the A operand by TMA multicast
   int lower_only;     // 1: skip tiles strictly above the block diagonal (GEMM(6))
   int mode;           // EpiMode
   // kEpiC: C[z * c_stride + row * ldc + col] (FP64)
   double* C;
   int64_t ldc, c_stride;
-  // kEpiX: row r = (q, i) = (r / nao, r % nao); X[i * ldx + q * x_cols + col]; running max of the
+  // kEpiX: row r = (q, i) = (r / nao, r % nao); X[r * ldx + col] (ldx = a_pad); running max of the
   // upper word of |X| per (group of q, i): xmax[qgroup[q] * nao + i]
   int nao;
   int x_cols;       // columns of X per q (a_pad); the N tiles of GEMM(5) cut this range
@@ -62,10 +63,12 @@ struct GemmProblem {
   // kEpiInt32: P[(w - 2) * a_rows * b_rows + row * b_rows + col] of flush chunk `dbg_chunk`
   int32_t* P;
   int dbg_chunk;
+  long long* dbg_clk;  // optional cycle counters of CTA 0 (timing experiments)
 };
 
 cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st);
 void set_gemm_debug_flags(int flags);
+void set_peak_tiles(int n);  // probe walks n distinct operand tiles (1 = the same tile every MMA)
 cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStream_t st);
 
 void set_jk_debug_flags(int flags);  // timing experiments: bit 0 = unpack writes nothing, bit 1 = reads nothing
@@ -81,11 +84,11 @@ cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const do
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
                                    int* status, cudaStream_t st);
-// X[i][col] (ldx) -> planes6[t][i][pitch6], e6[g][i]; col -> group by colgroup step: group g
-// covers columns [gcol[g], gcol[g+1]).
-cudaError_t launch_jk_split_x(const double* X, int nao, int64_t ncol, int64_t ldx, int s, int ng,
-                              const int* gcol, const uint32_t* xmax, int32_t* e6, int8_t* planes6,
-                              int64_t pitch6, int64_t plane_stride6, int* status, cudaStream_t st);
+// X[(q, i)][a_pad] -> planes6[t][i][q * a_pad + a] (pitch6), e6[g][i] from xmax; qgroup[q] = group of q.
+// planes6 bytes past nq * a_pad in a row are never read (TMA extent).
+cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int s, int ng, const int* qgroup,
+                              const uint32_t* xmax, int32_t* e6, int8_t* planes6, int64_t pitch6,
+                              int64_t plane_stride6, int* status, cudaStream_t st);
 // K (+)= sum_g Kpart[g] over lower block-triangle tiles (tile = 128), mirrored.
 cudaError_t launch_jk_k_reduce(const double* Kpart, int ng, int nao, int accumulate, double* K,
                                cudaStream_t st);

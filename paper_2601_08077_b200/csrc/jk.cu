@@ -215,46 +215,48 @@ __global__ void jk_x_scale_kernel(const uint32_t* __restrict__ xmax, long long n
   if (stt) atomicOr(status, stt);
 }
 
-// X[i][col] -> planes6[t][i][col]; a thread converts 16 consecutive columns (never straddling a
-// q, hence never a group, because a_pad is a multiple of 16).
+// X[(q, i)][a_pad] (GEMM(5)'s output, one contiguous 128-row block per tile) -> planes6[t][i][q * a_pad + a]
+// with the scale of (i, group of q).  A block owns one i and 32 consecutive q: it reads 32 runs of
+// a_pad doubles and writes one contiguous run of 32 * a_pad bytes per plane; a thread converts 16
+// consecutive columns.
 template <int S>
-__global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restrict__ X, int nao, long long ncol,
-                                                         long long ldx, int ng, const int* __restrict__ gcol,
+__global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restrict__ X, int nao, int nq, int a_pad,
+                                                         const int* __restrict__ qgroup,
                                                          const int32_t* __restrict__ e6,
                                                          int8_t* __restrict__ planes, long long pitch,
                                                          long long plane_stride) {
   const int i = blockIdx.y;
-  const long long run = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long c0 = run * 16;
-  if (c0 >= pitch) return;
-  uint32_t w[S][4];
+  const int runs_per_q = a_pad >> 4;
+  const int units = 32 * runs_per_q;
+  for (int u = threadIdx.x; u < units; u += blockDim.x) {
+    const int ql = u / runs_per_q, run = u - ql * runs_per_q;
+    const int q = blockIdx.x * 32 + ql;
+    if (q >= nq) break;
+    const double scale = pow2_double(63 - e6[(long long)qgroup[q] * nao + i]);
+    const double2* src = reinterpret_cast<const double2*>(X + ((long long)q * nao + i) * a_pad + run * 16);
+    double2 v[8];
 #pragma unroll
-  for (int t = 0; t < S; ++t)
+    for (int j = 0; j < 8; ++j) v[j] = __ldg(src + j);
+    uint32_t w[S][4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) w[t][j] = 0;
-  if (c0 < ncol) {
-    int lo = 0, hi = ng - 1;  // largest g with gcol[g] <= c0
-    while (lo < hi) {
-      const int mid = (lo + hi + 1) >> 1;
-      if (gcol[mid] <= c0) lo = mid; else hi = mid - 1;
-    }
-    const double scale = pow2_double(63 - e6[(long long)lo * nao + i]);
-    const double2* src = reinterpret_cast<const double2*>(X + (long long)i * ldx + c0);
+    for (int g4 = 0; g4 < 4; ++g4) {
+      uint32_t hi[4], lo[4];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      const double2 v = __ldg(src + j);
-      const uint64_t d0 = balanced_digits(v.x, scale), d1 = balanced_digits(v.y, scale);
-#pragma unroll
-      for (int t = 0; t < S; ++t) {
-        w[t][j >> 1] |= digit_byte(d0, t) << (8 * ((2 * j) & 3));
-        w[t][j >> 1] |= digit_byte(d1, t) << (8 * ((2 * j + 1) & 3));
+      for (int j = 0; j < 4; ++j) {
+        const double x = (j & 1) ? v[2 * g4 + (j >> 1)].y : v[2 * g4 + (j >> 1)].x;
+        const uint64_t dg = balanced_digits(x, scale);
+        hi[j] = (uint32_t)(dg >> 32);
+        lo[j] = (uint32_t)dg;
       }
-    }
-  }
 #pragma unroll
-  for (int t = 0; t < S; ++t)
-    *reinterpret_cast<uint4*>(planes + t * plane_stride + (long long)i * pitch + c0) =
-        make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+      for (int t = 0; t < S; ++t)
+        w[t][g4] = (t < 4) ? pack4_digit(hi[0], hi[1], hi[2], hi[3], 3 - t) : pack4_digit(lo[0], lo[1], lo[2], lo[3], 7 - t);
+    }
+#pragma unroll
+    for (int t = 0; t < S; ++t)
+      *reinterpret_cast<uint4*>(planes + t * plane_stride + (long long)i * pitch + (long long)q * a_pad + run * 16) =
+          make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+  }
 }
 
 // K[i][j] (+)= sum_g Kpart[g][i][j] for column tile <= row tile (tile = 128), mirrored to [j][i].
@@ -326,13 +328,13 @@ cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, 
   return cudaGetLastError();
 }
 
-cudaError_t launch_jk_split_x(const double* X, int nao, int64_t ncol, int64_t ldx, int s, int ng, const int* gcol,
+cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int s, int ng, const int* qgroup,
                               const uint32_t* xmax, int32_t* e6, int8_t* planes6, int64_t pitch6,
                               int64_t plane_stride6, int* status, cudaStream_t st) {
   const long long n = (long long)ng * nao;
   jk_x_scale_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(xmax, n, e6, status);
-  dim3 grid((unsigned)((pitch6 / 16 + 255) / 256), (unsigned)nao);
-  DFE_DISPATCH_S(s, (jk_split_x_kernel<SS><<<grid, 256, 0, st>>>(X, nao, ncol, ldx, ng, gcol, e6, planes6, pitch6,
+  dim3 grid((unsigned)((nq + 31) / 32), (unsigned)nao);
+  DFE_DISPATCH_S(s, (jk_split_x_kernel<SS><<<grid, 256, 0, st>>>(X, nao, nq, a_pad, qgroup, e6, planes6, pitch6,
                                                                  plane_stride6)));
   count_launch(2);
   return cudaGetLastError();

@@ -188,7 +188,7 @@ def run_jk(dfe, Bp, cfg_nao, naux, Cocc, nocc, D, s, want_x=True):
     a_pad = (nocc + 15) // 16 * 16
     J = torch.empty((cfg_nao, cfg_nao), dtype=torch.float64, device=DEV)
     K = torch.empty_like(J)
-    X = torch.zeros((cfg_nao, naux, a_pad), dtype=torch.float64, device=DEV) if want_x else None
+    X = torch.zeros((naux, cfg_nao, a_pad), dtype=torch.float64, device=DEV) if want_x else None
     e6 = torch.zeros((4096, cfg_nao), dtype=torch.int32, device=DEV)
     ng = dfe.df_debug_jk_build(dev(Bp), cfg_nao, naux, dev(Cocc), nocc, dev(D), s, J, K, X, e6)
     torch.cuda.synchronize()
@@ -206,7 +206,7 @@ def test_jk_tiny_config0(dfe, gpu_ws, tol):
     assert O.rel_frobenius(J, J_ref) <= 1e-12
     assert O.rel_frobenius(K, K_ref) <= tol
     # stage by stage: GEMM(5) output bit-exact, GEMM(6) scales exact, K up to FP64 summation order
-    assert np.array_equal(X[:, :, :cfg.nocc].transpose(1, 0, 2), X_emu)
+    assert np.array_equal(X[:, :, :cfg.nocc], X_emu)
     assert not X[:, :, cfg.nocc:].any()
     groups = O.q_groups(cfg.naux, cfg.nocc, s)
     assert ng == len(groups)
@@ -237,7 +237,7 @@ def test_jk_many_groups_and_superblocks(dfe, gpu_ws):
     K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
     J_ref, K_ref = O.df_jk_plain(Bp, nao, Cocc, D)
     assert ng == 5
-    assert np.array_equal(X[:, :, :nocc].transpose(1, 0, 2), X_emu)
+    assert np.array_equal(X[:, :, :nocc], X_emu)
     for g, (g0, g1) in enumerate(groups):
         Xrow = np.transpose(X_emu[g0:g1], (1, 0, 2)).reshape(nao, -1)
         assert np.array_equal(e6[g], O.scale_index(np.max(np.abs(Xrow), axis=1)))
@@ -264,7 +264,7 @@ def test_jk_split_n_tiles(dfe, gpu_ws, s):
     J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
     K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
     J_ref, K_ref = O.df_jk_plain(Bp, nao, Cocc, D)
-    assert np.array_equal(X[:, :, :nocc].transpose(1, 0, 2), X_emu)
+    assert np.array_equal(X[:, :, :nocc], X_emu)
     assert not X[:, :, nocc:].any()
     assert O.rel_frobenius(K, K_emu) <= 1e-14
     assert O.rel_frobenius(J, J_ref) <= 1e-12
@@ -311,7 +311,7 @@ def test_jk_medium_config2(dfe, gpu_ws):
         assert np.array_equal(K, K.T) and np.array_equal(J, J.T)
         for q in (0, 511, 512, 1699):
             Xq = O.emul_x_group(Bp, cfg.nao, Cocc, s, q, q + 1)[0]
-            assert np.array_equal(X[:, q, :cfg.nocc], Xq), f"q={q}"
+            assert np.array_equal(X[q, :, :cfg.nocc], Xq), f"q={q}"
     assert dfe.df_last_status() == 0
 
 
