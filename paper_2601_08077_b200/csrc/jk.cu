@@ -130,13 +130,6 @@ __global__ void __launch_bounds__(256) jk_j_gemv_kernel(const double* __restrict
   if (lane == 0) Jp[p] = acc;
 }
 
-// Four consecutive elements' digit words (upper or lower halves) -> the packed plane word of
-// digit byte `b` (0..3 within the half): three byte permutes instead of twelve shift/mask/or.
-__device__ __forceinline__ uint32_t pack4_digit(uint32_t h0, uint32_t h1, uint32_t h2, uint32_t h3, int b) {
-  const uint32_t sel = (uint32_t)b | ((uint32_t)(4 + b) << 4);
-  return __byte_perm(__byte_perm(h0, h1, sel), __byte_perm(h2, h3, sel), 0x5410);
-}
-
 // Unpack + split.  Output planes[t][(q, R)][C] want C-contiguous 128-byte lines, the input wants
 // q-contiguous runs.  A warp owns one output row R and 8 consecutive q; lane = (qi, cg): q = q8 + qi,
 // columns cg*32 .. cg*32+31 of a 128-column block.  One load instruction reads 64-byte runs of
@@ -221,7 +214,7 @@ __global__ void jk_x_scale_kernel(const uint32_t* __restrict__ xmax, long long n
 // consecutive columns.
 template <int S>
 __global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restrict__ X, int nao, int nq, int a_pad,
-                                                         const int* __restrict__ qgroup,
+                                                         int x_iq, const int* __restrict__ qgroup,
                                                          const int32_t* __restrict__ e6,
                                                          int8_t* __restrict__ planes, long long pitch,
                                                          long long plane_stride) {
@@ -233,7 +226,9 @@ __global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restric
     const int q = blockIdx.x * 32 + ql;
     if (q >= nq) break;
     const double scale = pow2_double(63 - e6[(long long)qgroup[q] * nao + i]);
-    const double2* src = reinterpret_cast<const double2*>(X + ((long long)q * nao + i) * a_pad + run * 16);
+    // X rows are (q, i) from the generic GEMM(5), (i, q) from the fused one
+    const long long xrow = x_iq ? (long long)i * nq + q : (long long)q * nao + i;
+    const double2* src = reinterpret_cast<const double2*>(X + xrow * a_pad + run * 16);
     double2 v[8];
 #pragma unroll
     for (int j = 0; j < 8; ++j) v[j] = __ldg(src + j);
@@ -328,13 +323,13 @@ cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, 
   return cudaGetLastError();
 }
 
-cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int s, int ng, const int* qgroup,
+cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int x_iq, int s, int ng, const int* qgroup,
                               const uint32_t* xmax, int32_t* e6, int8_t* planes6, int64_t pitch6,
                               int64_t plane_stride6, int* status, cudaStream_t st) {
   const long long n = (long long)ng * nao;
   jk_x_scale_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(xmax, n, e6, status);
   dim3 grid((unsigned)((nq + 31) / 32), (unsigned)nao);
-  DFE_DISPATCH_S(s, (jk_split_x_kernel<SS><<<grid, 256, 0, st>>>(X, nao, nq, a_pad, qgroup, e6, planes6, pitch6,
+  DFE_DISPATCH_S(s, (jk_split_x_kernel<SS><<<grid, 256, 0, st>>>(X, nao, nq, a_pad, x_iq, qgroup, e6, planes6, pitch6,
                                                                  plane_stride6)));
   count_launch(2);
   return cudaGetLastError();

@@ -257,7 +257,7 @@ def test_jk_split_n_tiles(dfe, gpu_ws, s):
     """nocc = 150 (config 3's value): a_pad = 160 does not fit s accumulators in TMEM, so GEMM(5)
     runs two N tiles of 80 columns (s = 4: one pass; s = 8: two passes with the FP64 read-modify-
     write); ragged nao, several M tiles straddling q boundaries."""
-    nao, naux, nocc = 168, 37, 150
+    nao, naux, nocc = 168, 38 if s == 4 else 37, 150  # even naux: fused GEMM(5); odd: separate unpack
     Bp = G.make_B_packed(nao, naux, seed=13)
     Cocc = G.make_C_occ(nao, nocc, seed=13)
     D = G.make_density(Cocc)
