@@ -158,11 +158,6 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
  * MMAs (operand feed only), bit 1 = issue no TMA loads (MMA issue only).  0 = normal. */
 int df_debug_set_gemm_flags(int flags);
 
-/* Cycle counters CTA 0 of the last GEMM(5) launch left in the workspace (timing experiments):
- * {epilogue wait, epilogue work, MMA-warp wait for operands, MMA-warp wait for TMEM, MMA-warp total}.
- * Synchronises the device. */
-int df_debug_read_clocks(int64_t* out8);
-
 /* Number of GPU kernels this library has launched in this process. */
 int64_t df_launch_count(void);
 

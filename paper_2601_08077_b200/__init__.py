@@ -15,7 +15,7 @@ _EXPORTS = (
     "df_emul_gemm_workspace_bytes", "df_jk_workspace_bytes", "df_jk_workspace_bytes_blocks", "df_set_workspace",
     "df_emul_gemm", "df_emul_gemm_slices", "df_jk_build", "df_jk_build_slices", "df_last_status",
     "df_debug_split_rows", "df_debug_split_cols", "df_debug_weight_sums", "df_debug_jk_build",
-    "df_debug_set_gemm_flags", "df_debug_read_clocks", "df_launch_count", "df_profile_enable", "df_profile_read", "df_debug_mma_peak",
+    "df_debug_set_gemm_flags", "df_launch_count", "df_profile_enable", "df_profile_read", "df_debug_mma_peak",
 )
 __all__ = list(_EXPORTS)
 

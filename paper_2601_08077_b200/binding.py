@@ -57,7 +57,6 @@ _SIG = {
     "df_debug_jk_build": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp, _vp,
                                  C.POINTER(C.c_int), _vp]),
     "df_debug_set_gemm_flags": (_i32, [_i32]),
-    "df_debug_read_clocks": (_i32, [C.POINTER(C.c_int64)]),
     "df_launch_count": (_i64, []),
     "df_profile_enable": (_i32, [_i32]),
     "df_profile_num_classes": (_i32, []),
@@ -226,12 +225,6 @@ def df_debug_jk_build(B_packed, nao, naux, C_occ, nocc, D, s, J, K, X_out=None, 
 
 def df_debug_set_gemm_flags(flags: int) -> None:
     _check(lib.df_debug_set_gemm_flags(int(flags)), "df_debug_set_gemm_flags")
-
-
-def df_debug_read_clocks():
-    out = (C.c_int64 * 8)()
-    _check(lib.df_debug_read_clocks(out), "df_debug_read_clocks")
-    return [int(x) for x in out]
 
 
 def df_launch_count() -> int:

@@ -22,7 +22,6 @@ static int g_mode = DF_MODE_GUARDED;
 static int g_device_ok = -1;
 static int g_g5_split_n = 1;
 static int g_g5_cluster = 1;
-static int g_g5_fused = 0;
 
 // ---- optional per-kernel-class CUDA-event timing (df_profile_*; bench.py's roofline) ----
 enum ProfClass { kPSplit = 0, kPPassA, kPJGemv, kPUnpack, kPGemm5, kPSplitX, kPGemm6, kPReduce, kPGemm, kPNum };
@@ -313,81 +312,51 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     DFE_CK(cudaMemsetAsync(w.xmax, 0, sizeof(uint32_t) * ng * nao, st));
 
     // the staging bulk copies need 16-byte aligned, 16-byte multiple runs of q: even naux and nq
-    const bool fused = g_g5_fused && gemm5_fused_supported((int)nao, w.a_pad, s) && naux % 2 == 0 && nq % 2 == 0;
-    if (fused) {
-      // H1/H2/H3/H4 in one kernel: packed FP64 B -> digits in shared memory -> MMAs -> X[i][q][a]
-      ProfScope ps(kPGemm5, st);
-      Gemm5FusedProblem f5 = {};
-      f5.Bp = Bp;
-      f5.emax = w.emax5;
-      f5.planesC = w.pc;
-      f5.eC = w.eC;
-      f5.c_pitch = w.pitchj;
-      f5.c_plane_stride = (int64_t)w.a_pad * w.pitchj;
-      f5.X = w.X;
-      f5.qgroup = w.qgroup;
-      f5.xmax = w.xmax;
-      f5.status = w.status;
-      f5.nao = (int)nao;
-      f5.naux = (int)naux;
-      f5.qs0 = (int)qs0;
-      f5.nq = nq;
-      f5.a_pad = w.a_pad;
-      f5.s = s;
-      DFE_CK(launch_gemm5_fused(f5, st));
-      if (X_out)
-        for (int64_t i = 0; i < nao; ++i)
-          DFE_CK(cudaMemcpy2DAsync(X_out + (qs0 * nao + i) * w.a_pad, sizeof(double) * nao * w.a_pad,
-                                   w.X + i * nq * w.a_pad, sizeof(double) * w.a_pad, sizeof(double) * w.a_pad, nq,
-                                   cudaMemcpyDeviceToDevice, st));
-    } else {
-      // H2: unpack + split packed B -> planes5 rows (q, i), contraction j
-      {
-        ProfScope ps(kPUnpack, st);
-        DFE_CK(launch_jk_unpack_split(Bp, (int)nao, (int)naux, (int)qs0, (int)qs1, w.emax5, s, w.e5, w.p5,
-                                      w.pitchj, (int64_t)nq * nao * w.pitchj, w.status, st));
-      }
-      // GEMM(5): X[i][q][a] = sum_j B^q_ij C_ja   (Eq. 5 / Eq. 12)
-      GemmProblem g5 = {};
-      g5.A = w.p5;
-      g5.B = w.pc;
-      g5.a_rows = (int64_t)nq * nao;
-      g5.b_rows = w.a_pad;
-      g5.k = nao;
-      g5.a_pitch = g5.b_pitch = w.pitchj;
-      g5.a_plane_stride = (int64_t)nq * nao * w.pitchj;
-      g5.b_plane_stride = (int64_t)w.a_pad * w.pitchj;
-      g5.s = s;
-      // N tile: the whole a_pad when all s weight accumulators fit TMEM (s * a_pad <= 512 columns),
-      // else half of it, so that X is written once instead of read-modify-written per pass
-      g5.n_tile = w.a_pad;
-      if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) g5.n_tile = w.a_pad / 2;
-      g5.acc_stride = (g5.n_tile % 32) ? g5.n_tile : 0;
-      g5.x_cols = w.a_pad;
-      g5.cluster_n = (g_g5_cluster && g5.n_tile * 2 == w.a_pad) ? 2 : 1;
-      g5.nz = 1;
-      g5.eA = w.e5;
-      g5.eB = w.eC;
-      g5.mode = kEpiX;
-      g5.C = w.X;
-      g5.nao = (int)nao;
-      g5.ldx = w.a_pad;
-      g5.qgroup = w.qgroup;
-      g5.xmax = w.xmax;
-      g5.dbg_clk = (long long*)(w.status + 16);  // 8 counters inside the 256-byte status block
-      {
-        ProfScope ps(kPGemm5, st);
-        DFE_CK(launch_gemm_i8(g5, st));
-      }
-      if (X_out)
-        DFE_CK(cudaMemcpyAsync(X_out + qs0 * nao * w.a_pad, w.X, sizeof(double) * nq * nao * w.a_pad,
-                               cudaMemcpyDeviceToDevice, st));
+    // H2: unpack + split packed B -> planes5 rows (q, i), contraction j
+    {
+      ProfScope ps(kPUnpack, st);
+      DFE_CK(launch_jk_unpack_split(Bp, (int)nao, (int)naux, (int)qs0, (int)qs1, w.emax5, s, w.e5, w.p5,
+                                    w.pitchj, (int64_t)nq * nao * w.pitchj, w.status, st));
     }
+    // GEMM(5): X[i][q][a] = sum_j B^q_ij C_ja   (Eq. 5 / Eq. 12)
+    GemmProblem g5 = {};
+    g5.A = w.p5;
+    g5.B = w.pc;
+    g5.a_rows = (int64_t)nq * nao;
+    g5.b_rows = w.a_pad;
+    g5.k = nao;
+    g5.a_pitch = g5.b_pitch = w.pitchj;
+    g5.a_plane_stride = (int64_t)nq * nao * w.pitchj;
+    g5.b_plane_stride = (int64_t)w.a_pad * w.pitchj;
+    g5.s = s;
+    // N tile: the whole a_pad when all s weight accumulators fit TMEM (s * a_pad <= 512 columns),
+    // else half of it, so that X is written once instead of read-modify-written per pass
+    g5.n_tile = w.a_pad;
+    if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) g5.n_tile = w.a_pad / 2;
+    g5.acc_stride = (g5.n_tile % 32) ? g5.n_tile : 0;
+    g5.x_cols = w.a_pad;
+    g5.cluster_n = (g_g5_cluster && g5.n_tile * 2 == w.a_pad) ? 2 : 1;
+    g5.nz = 1;
+    g5.eA = w.e5;
+    g5.eB = w.eC;
+    g5.mode = kEpiX;
+    g5.C = w.X;
+    g5.nao = (int)nao;
+    g5.ldx = w.a_pad;
+    g5.qgroup = w.qgroup;
+    g5.xmax = w.xmax;
+      {
+      ProfScope ps(kPGemm5, st);
+      DFE_CK(launch_gemm_i8(g5, st));
+    }
+    if (X_out)
+      DFE_CK(cudaMemcpyAsync(X_out + qs0 * nao * w.a_pad, w.X, sizeof(double) * nq * nao * w.a_pad,
+                             cudaMemcpyDeviceToDevice, st));
 
     // X -> planes6 with one scale per (i, group)
     {
       ProfScope ps(kPSplitX, st);
-      DFE_CK(launch_jk_split_x(w.X, (int)nao, nq, w.a_pad, fused ? 1 : 0, s, ng, w.qgroup, w.xmax, w.e6, w.p6, pitch6,
+      DFE_CK(launch_jk_split_x(w.X, (int)nao, nq, w.a_pad, s, ng, w.qgroup, w.xmax, w.e6, w.p6, pitch6,
                                (int64_t)nao * pitch6, w.status, st));
     }
     if (e6_out)
@@ -593,16 +562,8 @@ int df_debug_set_gemm_flags(int flags) {
   set_gemm_debug_flags(flags);
   g_g5_split_n = (flags & 4) ? 0 : 1;
   g_g5_cluster = (flags & 64) ? 0 : 1;
-  g_g5_fused = (flags & 128) ? 1 : 0;    // bit 7: experimental fused unpack+split+GEMM(5) kernel  // bit 6: GEMM(5) without the cluster-pair multicast
   set_jk_debug_flags((flags >> 4) & 3);
   set_peak_tiles((flags >> 16) & 15);  // bits 16,17: MMA probe walks 1..4 operand tiles; bits 18,19: swizzle 32/64/128  // bits 4, 5: unpack kernel without stores / without loads  // bit 2: GEMM(5) keeps one N tile (multi-pass read-modify-write)
-  return DF_OK;
-}
-
-int df_debug_read_clocks(int64_t* out8) {
-  if (!out8) return DF_ERR_NULL;
-  if (!g_ws) return DF_ERR_WORKSPACE;
-  if (cudaMemcpy(out8, (char*)g_ws + 64, 8 * sizeof(int64_t), cudaMemcpyDeviceToHost) != cudaSuccess) return DF_ERR_CUDA;
   return DF_OK;
 }
 

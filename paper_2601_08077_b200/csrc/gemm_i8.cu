@@ -56,7 +56,6 @@ struct GemmKernelParams {
   // [pass_start[ps], pass_start[ps+1])
   uint2 pairs[kMaxSlices * (kMaxSlices + 1) / 2];
   int pass_start[kMaxSlices + 1];
-  long long* dbg_clk;  // optional: cycles of CTA 0 {epilogue wait, epilogue work, MMA-warp wait, MMA-warp issue, producer wait}
   int dbg_flags;  // bit 0: no MMAs (operand feed only); bit 1: no TMA loads (MMA issue only)
 };
 
@@ -210,8 +209,6 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     const uint32_t smem_base16 = (smem_u32(smem) & 0x3FFFFu) >> 4;
     const uint32_t stage16 = p.stage_stride >> 4;
     uint32_t it = 0, iter = 0;
-    long long clk_mwait = 0, clk_tmem = 0;
-    const long long clk_m0 = clock64();
     DFE_WORK_LOOP
     for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
       const int kc0 = zk0 + ch * p.kflush;
@@ -220,18 +217,14 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
       for (int ps = 0; ps < npass; ++ps, ++iter) {
         const int pr0 = p.pass_start[ps], pr1 = p.pass_start[ps + 1];
         if (iter > 0) {
-          const long long tt0 = clock64();
           mbar_wait(&tmem_empty_bar, (iter - 1) & 1u);
           tc_fence_after();
-          clk_tmem += clock64() - tt0;
         }
         for (int kb = 0; kb < nkb; ++kb, ++it) {
           const uint32_t stage = it % S;
           const uint32_t ph = (it / S) & 1u;
-          const long long tw0 = clock64();
           mbar_wait(&full_bar[stage], ph);
           tc_fence_after();
-          clk_mwait += clock64() - tw0;
           if (p.dbg_flags & 1) {
             if (lane == 0) mbar_arrive(&empty_bar[stage]);
             continue;
@@ -263,16 +256,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
       }
     }
     }  // work loop
-    if (p.dbg_clk && blockIdx.x == 0 && lane == 0) {
-      p.dbg_clk[2] = clk_mwait;
-      p.dbg_clk[3] = clk_tmem;
-      p.dbg_clk[4] = clock64() - clk_m0;
-    }
   } else {
     // ================= epilogue: TMEM -> FP64 recombination -> global =================
     const int quarter = warp & 3;
     uint32_t iter = 0;
-    long long clk_wait = 0, clk_work = 0;
     DFE_WORK_LOOP
     const int row_local = quarter * 32 + lane;
     const long long row = (long long)tm * kTileM + row_local;
@@ -316,11 +303,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         pass_weights(s, W, ps, w_hi, w_lo);
         const bool first = (ch == chunk_lo) && (ps == 0);
         const bool last = (ch == chunk_hi - 1) && (ps == npass - 1);
-        const long long t0 = clock64();
         mbar_wait(&tmem_full_bar, iter & 1u);
         tc_fence_after();
-        const long long t1 = clock64();
-        clk_wait += t1 - t0;
         for (int c = chalf * 16; c < p.n_tile; c += 32) {
           uint32_t v[16];
           if (p.mode == kEpiInt32) {
@@ -415,7 +399,6 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         }
         tc_fence_before();
         mbar_arrive(&tmem_empty_bar);
-        clk_work += clock64() - t1;
       }
     }
     if (p.mode == kEpiX && row_ok) {
@@ -424,10 +407,6 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
       atomicMax(&p.xmax[(long long)p.qgroup[q] * p.nao + i], hi_max);
     }
     }  // work loop
-    if (p.dbg_clk && blockIdx.x == 0 && warp == 2 && lane == 0) {
-      p.dbg_clk[0] = clk_wait;
-      p.dbg_clk[1] = clk_work;
-    }
   }
 
   tc_fence_before();
@@ -454,7 +433,7 @@ __global__ void __launch_bounds__(128, 1) mma_peak_kernel(int n_mma, int iters, 
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t done_bar;
   __shared__ uint32_t tmem_slot;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = threadIdx.x >> 5;
   // ntiles A tiles of 128 rows x 32 B (SW32, 4 KB each) and ntiles B tiles of 256 rows x 32 B,
   // zero-filled; ntiles > 1 walks different tiles so that no operand can be reused from the
   // previous MMA (shared-memory operand bandwidth shows).
@@ -647,7 +626,6 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.P = g.P;
   p.dbg_chunk = g.dbg_chunk;
   p.dbg_flags = g_gemm_dbg_flags;
-  p.dbg_clk = g.dbg_clk;
 
   p.tiles_per_z = g.lower_only ? p.tiles_m * (p.tiles_m + 1) / 2 : p.tiles_m * p.tiles_n;
   p.total_work = (long long)p.tiles_per_z * g.nz;

@@ -63,7 +63,6 @@ struct GemmProblem {
   // kEpiInt32: P[(w - 2) * a_rows * b_rows + row * b_rows + col] of flush chunk `dbg_chunk`
   int32_t* P;
   int dbg_chunk;
-  long long* dbg_clk;  // optional cycle counters of CTA 0 (timing experiments)
 };
 
 cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st);
@@ -72,23 +71,6 @@ void set_peak_tiles(int n);  // probe walks n distinct operand tiles (1 = the sa
 cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStream_t st);
 
 void set_jk_debug_flags(int flags);  // timing experiments: bit 0 = unpack writes nothing, bit 1 = reads nothing
-// ---- gemm5_fused.cu --------------------------------------------------------
-// GEMM(5) with the unpack + split of packed B fused into the operand producer (cluster pairs).
-struct Gemm5FusedProblem {
-  const double* Bp;          // packed B [npair][naux]
-  const uint32_t* emax;      // [nao][naux]
-  const int8_t* planesC;     // [s][a_pad][c_pitch] C_occ digit planes (K-major), scales eC[a_pad]
-  const int32_t* eC;
-  int64_t c_pitch, c_plane_stride;
-  double* X;                 // out: [nao][nq][a_pad]
-  const int* qgroup;         // [nq]
-  uint32_t* xmax;            // [group][nao], zeroed by the caller
-  int* status;
-  int nao, naux, qs0, nq, a_pad, s;
-};
-bool gemm5_fused_supported(int nao, int a_pad, int s);
-cudaError_t launch_gemm5_fused(const Gemm5FusedProblem& g, cudaStream_t st);
-
 // ---- jk.cu ----------------------------------------------------------------
 // pass A over packed B: rho[q] (+=, must be zeroed) and emax[i * naux + q] = upper word of
 // max_j |B^q_ij| (atomicMax, must be zeroed).
@@ -101,9 +83,9 @@ cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const do
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
                                    int* status, cudaStream_t st);
-// X[(q, i)][a_pad] (x_iq = 0) or X[(i, q)][a_pad] (x_iq = 1) -> planes6[t][i][q * a_pad + a] (pitch6), e6[g][i] from xmax; qgroup[q] = group of q.
+// X[(q, i)][a_pad] -> planes6[t][i][q * a_pad + a] (pitch6), e6[g][i] from xmax; qgroup[q] = group of q.
 // planes6 bytes past nq * a_pad in a row are never read (TMA extent).
-cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int x_iq, int s, int ng, const int* qgroup,
+cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int s, int ng, const int* qgroup,
                               const uint32_t* xmax, int32_t* e6, int8_t* planes6, int64_t pitch6,
                               int64_t plane_stride6, int* status, cudaStream_t st);
 // K (+)= sum_g Kpart[g] over lower block-triangle tiles (tile = 128), mirrored.

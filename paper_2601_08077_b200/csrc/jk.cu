@@ -214,7 +214,7 @@ __global__ void jk_x_scale_kernel(const uint32_t* __restrict__ xmax, long long n
 // consecutive columns.
 template <int S>
 __global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restrict__ X, int nao, int nq, int a_pad,
-                                                         int x_iq, const int* __restrict__ qgroup,
+                                                         const int* __restrict__ qgroup,
                                                          const int32_t* __restrict__ e6,
                                                          int8_t* __restrict__ planes, long long pitch,
                                                          long long plane_stride) {
@@ -226,9 +226,7 @@ __global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restric
     const int q = blockIdx.x * 32 + ql;
     if (q >= nq) break;
     const double scale = pow2_double(63 - e6[(long long)qgroup[q] * nao + i]);
-    // X rows are (q, i) from the generic GEMM(5), (i, q) from the fused one
-    const long long xrow = x_iq ? (long long)i * nq + q : (long long)q * nao + i;
-    const double2* src = reinterpret_cast<const double2*>(X + xrow * a_pad + run * 16);
+    const double2* src = reinterpret_cast<const double2*>(X + ((long long)q * nao + i) * a_pad + run * 16);
     double2 v[8];
 #pragma unroll
     for (int j = 0; j < 8; ++j) v[j] = __ldg(src + j);
@@ -323,13 +321,13 @@ cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, 
   return cudaGetLastError();
 }
 
-cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int x_iq, int s, int ng, const int* qgroup,
+cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int s, int ng, const int* qgroup,
                               const uint32_t* xmax, int32_t* e6, int8_t* planes6, int64_t pitch6,
                               int64_t plane_stride6, int* status, cudaStream_t st) {
   const long long n = (long long)ng * nao;
   jk_x_scale_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(xmax, n, e6, status);
   dim3 grid((unsigned)((nq + 31) / 32), (unsigned)nao);
-  DFE_DISPATCH_S(s, (jk_split_x_kernel<SS><<<grid, 256, 0, st>>>(X, nao, nq, a_pad, x_iq, qgroup, e6, planes6, pitch6,
+  DFE_DISPATCH_S(s, (jk_split_x_kernel<SS><<<grid, 256, 0, st>>>(X, nao, nq, a_pad, qgroup, e6, planes6, pitch6,
                                                                  plane_stride6)));
   count_launch(2);
   return cudaGetLastError();
