@@ -311,7 +311,6 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     DFE_CK(cudaGetLastError());
     DFE_CK(cudaMemsetAsync(w.xmax, 0, sizeof(uint32_t) * ng * nao, st));
 
-    // the staging bulk copies need 16-byte aligned, 16-byte multiple runs of q: even naux and nq
     // H2: unpack + split packed B -> planes5 rows (q, i), contraction j
     {
       ProfScope ps(kPUnpack, st);
