@@ -328,8 +328,10 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     g5.a_plane_stride = (int64_t)nq * nao * w.pitchj;
     g5.b_plane_stride = (int64_t)w.a_pad * w.pitchj;
     g5.s = s;
-    // N tile: the whole a_pad when all s weight accumulators fit TMEM (s * a_pad <= 512 columns),
-    // else half of it, so that X is written once instead of read-modify-written per pass
+    // N tile: the whole a_pad when all s weight accumulators fit TMEM (s * a_pad <= 512 columns), else
+    // two halves on a CTA pair that shares the A operand by multicast (measured at nocc = 150:
+    // 12.6 / 15.9 / 20.5 ms at s = 4 / 5 / 6 against 13.8 / 19.8 / 26.8 ms for one 160-column tile
+    // in two or more passes -- N = 160 MMAs are shared-memory-bandwidth bound)
     g5.n_tile = w.a_pad;
     if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) g5.n_tile = w.a_pad / 2;
     g5.acc_stride = (g5.n_tile % 32) ? g5.n_tile : 0;
@@ -559,7 +561,7 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t 
 
 int df_debug_set_gemm_flags(int flags) {
   set_gemm_debug_flags(flags);
-  g_g5_split_n = (flags & 4) ? 0 : 1;
+  g_g5_split_n = (flags & 4) ? 0 : 1;  // bit 2: GEMM(5) keeps one N tile
   g_g5_cluster = (flags & 64) ? 0 : 1;
   set_jk_debug_flags((flags >> 4) & 3);
   set_peak_tiles((flags >> 16) & 15);  // bits 16,17: MMA probe walks 1..4 operand tiles; bits 18,19: swizzle 32/64/128  // bits 4, 5: unpack kernel without stores / without loads  // bit 2: GEMM(5) keeps one N tile (multi-pass read-modify-write)

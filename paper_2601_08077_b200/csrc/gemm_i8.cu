@@ -31,6 +31,11 @@ struct GemmKernelParams {
   CUtensorMap mapB;
   CUtensorMap mapA2;  // A planes with a 64-row box (cluster pair: each CTA loads and multicasts half a tile)
   int s, n_tile, acc_stride, weights_per_pass;
+  // pass structure: weights_per_pass weights in pass 0; tp = 1 ("TMEM partial"): the FP64 running
+  // sum stays in TMEM between passes (low words in accumulator slot 0, high words in slot 1) and
+  // later passes use slots 2.. (weights_later each); tp = 0: every pass takes weights_per_pass and
+  // the running sum is read-modify-written in global memory
+  int tp, weights_later, npass;
   int tiles_m, tiles_n, group_m, tiles_per_z;
   long long total_work;
   int num_stages;
@@ -59,10 +64,18 @@ struct GemmKernelParams {
   int dbg_flags;  // bit 0: no MMAs (operand feed only); bit 1: no TMA loads (MMA issue only)
 };
 
-// weights of pass `ps`: w_hi down to w_lo
-__device__ __forceinline__ void pass_weights(int s, int W, int ps, int& w_hi, int& w_lo) {
-  w_hi = s + 1 - ps * W;
-  w_lo = max(2, w_hi - W + 1);
+// weights of pass `ps`: w_hi down to w_lo; weight w accumulates in TMEM slot slot0 + (w_hi - w)
+__device__ __forceinline__ void pass_weights(const GemmKernelParams& p, int ps, int& w_hi, int& w_lo, int& slot0) {
+  const int W = p.weights_per_pass;
+  if (!p.tp || ps == 0) {
+    w_hi = p.s + 1 - ps * W;
+    w_lo = max(2, w_hi - W + 1);
+    slot0 = 0;
+  } else {
+    w_hi = p.s + 1 - W - (ps - 1) * p.weights_later;
+    w_lo = max(2, w_hi - p.weights_later + 1);
+    slot0 = 2;
+  }
 }
 
 // One unit of work of the persistent kernel: an output tile of one z item.
@@ -126,8 +139,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
   const int s = p.s;
-  const int W = p.weights_per_pass;
-  const int npass = (s + W - 1) / W;
+  const int npass = p.npass;
   const int S = p.num_stages;
   // CL == 2: a cluster of two CTAs owns the two N tiles of one M tile (work items 2c, 2c+1); each
   // loads half of every A plane tile and multicasts it to both, so the A operand crosses L2 once.
@@ -166,8 +178,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         const int kc1 = min(zk1, kc0 + p.kflush);
         const int nkb = (kc1 - kc0 + BK - 1) / BK;
         for (int ps = 0; ps < npass; ++ps) {
-          int w_hi, w_lo;
-          pass_weights(s, W, ps, w_hi, w_lo);
+          int w_hi, w_lo, slot0;
+          pass_weights(p, ps, w_hi, w_lo, slot0);
           const int P = min(s, w_hi - 1);
           const uint32_t tx = (uint32_t)P * (a_plane_bytes + b_plane_bytes);
           for (int kb = 0; kb < nkb; ++kb, ++it) {
@@ -299,8 +311,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     uint32_t hi_max = 0;
     for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
       for (int ps = 0; ps < npass; ++ps, ++iter) {
-        int w_hi, w_lo;
-        pass_weights(s, W, ps, w_hi, w_lo);
+        int w_hi, w_lo, slot0;
+        pass_weights(p, ps, w_hi, w_lo, slot0);
         const bool first = (ch == chunk_lo) && (ps == 0);
         const bool last = (ch == chunk_hi - 1) && (ps == npass - 1);
         mbar_wait(&tmem_full_bar, iter & 1u);
@@ -309,7 +321,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
           uint32_t v[16];
           if (p.mode == kEpiInt32) {
             for (int w = w_hi; w >= w_lo; --w) {
-              tmem_ld16(t_lane + (uint32_t)((w_hi - w) * p.acc_stride + c), v);
+              tmem_ld16(t_lane + (uint32_t)((slot0 + w_hi - w) * p.acc_stride + c), v);
               tmem_ld_wait();
               if (row_ok) {
 #pragma unroll
@@ -329,7 +341,15 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             eBv[j] = (row_ok && col < p.b_rows) ? p.eB[z * p.eb_stride + col] : 0;
             acc[j] = 0.0;
           }
-          if (!first) {
+          if (!first && p.tp) {
+            // running sum of the earlier passes: low words in slot 0, high words in slot 1
+            uint32_t plo[16];
+            tmem_ld16(t_lane + (uint32_t)c, plo);
+            tmem_ld16(t_lane + (uint32_t)(p.acc_stride + c), v);
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) acc[j] = __hiloint2double((int)v[j], (int)plo[j]);
+          } else if (!first) {
             // running sum of the earlier passes/chunks: coalesced 16-byte loads (4 lanes cover 64
             // bytes of a row), transposed through shared memory to "lane = row"
             if (vec_ok) {
@@ -361,7 +381,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             }
           }
           for (int w = w_hi; w >= w_lo; --w) {
-            tmem_ld16(t_lane + (uint32_t)((w_hi - w) * p.acc_stride + c), v);
+            tmem_ld16(t_lane + (uint32_t)((slot0 + w_hi - w) * p.acc_stride + c), v);
             tmem_ld_wait();
             const int eb = eA + 2 - 8 * w;
 #pragma unroll
@@ -373,7 +393,17 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             for (int j = 0; j < 16; ++j)
               if (col0 + c + j < p.b_rows) hi_max = max(hi_max, abs_hi_word(acc[j]));
           }
-          if (vec_ok) {
+          if (p.tp && !last) {
+            // park the running sum in TMEM (the columns this block of slots 0 and 1 just gave up)
+            uint32_t plo[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+              plo[j] = (uint32_t)__double2loint(acc[j]);
+              v[j] = (uint32_t)__double2hiint(acc[j]);
+            }
+            tmem_st16(t_lane + (uint32_t)c, plo);
+            tmem_st16(t_lane + (uint32_t)(p.acc_stride + c), v);
+          } else if (vec_ok) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
               const long long colv = col0 + c + 8 * h + cpair;
@@ -397,6 +427,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             }
           }
         }
+        if (p.tp && !last) tmem_st_wait();
         tc_fence_before();
         mbar_arrive(&tmem_empty_bar);
       }
@@ -541,8 +572,10 @@ static uint32_t stage_stride_for(int s, int n_tile, int bk) {
 
 static int g_gemm_dbg_flags = 0;
 static int g_gemm_force_bk = 0;
+static int g_gemm_no_tp = 0;
 void set_gemm_debug_flags(int flags) {
   g_gemm_dbg_flags = flags & 3;
+  g_gemm_no_tp = (flags >> 3) & 1;  // bit 3: multi-pass through global read-modify-write instead of TMEM
   const int f = (flags >> 8) & 0xFF;  // bits 8..15: force the K-block width (32, 64, 128; 0 = auto)
   g_gemm_force_bk = (f == 32 || f == 64 || f == 128) ? f : 0;
 }
@@ -571,15 +604,42 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.s = s;
   p.n_tile = g.n_tile;
   p.acc_stride = g.acc_stride > 0 ? g.acc_stride : (int)round_up(g.n_tile, 32);
-  p.weights_per_pass = 512 / p.acc_stride;
-  if (p.weights_per_pass > s) p.weights_per_pass = s;
   {
-    const int W = p.weights_per_pass, npass = (s + W - 1) / W;
+    const int W0 = 512 / p.acc_stride;  // accumulator slots in TMEM
+    const bool one_chunk = g.zk != nullptr || g.k <= kflush_for(s);  // q-groups fit one chunk by construction
+    p.tp = 0;
+    p.weights_later = 0;
+    if (s <= W0) {
+      p.weights_per_pass = s;
+      p.npass = 1;
+    } else if (W0 >= 3 && one_chunk && g.mode != kEpiInt32 && !g_gemm_no_tp &&
+               1 + (s - W0 + W0 - 3) / (W0 - 2) <= (s + W0 - 1) / W0) {
+      // park the running sum in TMEM when that costs no extra pass over the contraction
+      p.tp = 1;
+      p.weights_per_pass = W0;
+      p.weights_later = W0 - 2;
+      p.npass = 1 + (s - W0 + p.weights_later - 1) / p.weights_later;
+    } else {
+      p.weights_per_pass = W0;
+      p.npass = (s + W0 - 1) / W0;
+    }
+  }
+  {
+    const int npass = p.npass;
     const uint32_t a_plane = (uint32_t)kTileM * bk, b_plane = (uint32_t)g.n_tile * bk, b_off = (uint32_t)s * a_plane;
     int np = 0;
     for (int ps = 0; ps < npass; ++ps) {
       p.pass_start[ps] = np;
-      const int w_hi = s + 1 - ps * W, w_lo = (w_hi - W + 1) > 2 ? (w_hi - W + 1) : 2;
+      int w_hi, w_lo, slot0 = 0;
+      if (!p.tp || ps == 0) {
+        w_hi = s + 1 - ps * p.weights_per_pass;
+        w_lo = w_hi - p.weights_per_pass + 1;
+      } else {
+        w_hi = s + 1 - p.weights_per_pass - (ps - 1) * p.weights_later;
+        w_lo = w_hi - p.weights_later + 1;
+        slot0 = 2;
+      }
+      if (w_lo < 2) w_lo = 2;
       // round-robin over the weights of the pass, so that consecutive MMAs target different TMEM
       // accumulators (back-to-back MMAs into one accumulator wait on each other)
       int next_t[kMaxSlices + 2];
@@ -594,7 +654,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
           next_t[w] = t + 1;
           const uint32_t ao = ((uint32_t)(t - 1) * a_plane) >> 4, bo = (b_off + (uint32_t)(w - t - 1) * b_plane) >> 4;
           p.pairs[np].x = ao | (bo << 16);
-          p.pairs[np].y = (uint32_t)((w_hi - w) * p.acc_stride) | ((t > t_lo ? 1u : 0u) << 16);
+          p.pairs[np].y = (uint32_t)((slot0 + w_hi - w) * p.acc_stride) | ((t > t_lo ? 1u : 0u) << 16);
           ++np;
         }
       }
