@@ -170,6 +170,7 @@ static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m
   g.eA = w.eA;
   g.eB = w.eB;
   g.mode = kEpiC;
+  g.pair = 1;
   g.C = C;
   g.ldc = n;
   {
@@ -380,6 +381,7 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     g6.eB = w.e6;
     g6.ea_stride = g6.eb_stride = nao;
     g6.lower_only = 1;
+    g6.pair = 1;
     g6.mode = kEpiC;
     g6.C = w.Kpart;
     g6.ldc = nao;

@@ -29,6 +29,7 @@ constexpr int kSmemLimit = 232448 - 21504;  // 227 KB minus the static shared me
 struct GemmKernelParams {
   CUtensorMap mapA;
   CUtensorMap mapB;
+  CUtensorMap mapBh;  // B planes with a 64-row box (cta_group::2 pair: each CTA holds half of the N rows)
   CUtensorMap mapA2;  // A planes with a 64-row box (cluster pair: each CTA loads and multicasts half a tile)
   int s, n_tile, acc_stride, weights_per_pass;
   // pass structure: weights_per_pass weights in pass 0; tp = 1 ("TMEM partial"): the FP64 running
@@ -36,7 +37,7 @@ struct GemmKernelParams {
   // later passes use slots 2.. (weights_later each); tp = 0: every pass takes weights_per_pass and
   // the running sum is read-modify-written in global memory
   int tp, weights_later, npass;
-  int tiles_m, tiles_n, group_m, tiles_per_z;
+  int tiles_m, tiles_n, group_m, tiles_per_z, pair;
   long long total_work;
   int num_stages;
   uint32_t stage_stride;
@@ -89,7 +90,14 @@ __device__ __forceinline__ WorkItem decode_work(const GemmKernelParams& p, long 
   WorkItem w;
   w.z = (int)(wi / p.tiles_per_z);
   const int lin = (int)(wi - (long long)w.z * p.tiles_per_z);
-  if (p.lower_only) {
+  if (p.lower_only && p.pair) {
+    // pairs of M tiles (256 rows) against N tiles of 128: tn <= 2 tm2 + 1; a(a+1) items precede row a
+    int a = (int)((sqrtf(4.0f * (float)lin + 1.0f) - 1.0f) * 0.5f);
+    while ((a + 1) * (a + 2) <= lin) ++a;
+    while (a * (a + 1) > lin) --a;
+    w.tm = a;
+    w.tn = lin - a * (a + 1);
+  } else if (p.lower_only) {
     int a = (int)((sqrtf(8.0f * (float)lin + 1.0f) - 1.0f) * 0.5f);
     while ((a + 1) * (a + 2) / 2 <= lin) ++a;
     while (a * (a + 1) / 2 > lin) --a;
@@ -116,10 +124,14 @@ __device__ __forceinline__ WorkItem decode_work(const GemmKernelParams& p, long 
 }
 
 #define DFE_WORK_LOOP                                                                  \
-  for (long long wi = (CL == 1) ? (long long)blockIdx.x : (long long)(blockIdx.x & ~1u) + crank; wi < p.total_work;  \
-       wi += gridDim.x) {                                                              \
+  for (long long wi = (CL == 1) ? (long long)blockIdx.x                                \
+                      : (CL == 2) ? (long long)(blockIdx.x & ~1u) + crank              \
+                                  : (long long)(blockIdx.x >> 1);                      \
+       wi < p.total_work; wi += (CL == 4) ? (gridDim.x >> 1) : gridDim.x) {            \
     const WorkItem wk = decode_work(p, wi);                                            \
-    const int tm = wk.tm, tn = wk.tn, z = wk.z, zk0 = wk.zk0, zk1 = wk.zk1;            \
+    if (CL == 4 && wk.tn >= p.tiles_n) continue; /* ragged last pair row, lower_only */ \
+    const int tm = (CL == 4) ? 2 * wk.tm + (int)crank : wk.tm;                         \
+    const int tn = wk.tn, z = wk.z, zk0 = wk.zk0, zk1 = wk.zk1;                        \
     const int chunk_lo = wk.chunk_lo, chunk_hi = wk.chunk_hi;                          \
     (void)tm; (void)tn; (void)z; (void)zk0; (void)zk1;
 
@@ -143,7 +155,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   const int S = p.num_stages;
   // CL == 2: a cluster of two CTAs owns the two N tiles of one M tile (work items 2c, 2c+1); each
   // loads half of every A plane tile and multicasts it to both, so the A operand crosses L2 once.
-  const uint32_t crank = (CL == 2) ? cluster_ctarank() : 0u;
+  // CL == 4: the pair runs cta_group::2 MMAs of M = 256: CTA r owns rows 128 r .. 128 r + 127 of the
+  // 256-row tile and holds N rows 64 r .. 64 r + 63 of every B plane tile; CTA 0 issues.
+  const uint32_t crank = (CL != 1) ? cluster_ctarank() : 0u;
   (void)crank;
 
   if (warp == 0 && lane == 0) {
@@ -151,21 +165,24 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     prefetch_tensormap(&p.mapB);
     for (int i = 0; i < S; ++i) {
       mbar_init(&full_bar[i], 1);
-      mbar_init(&empty_bar[i], CL);
+      mbar_init(&empty_bar[i], CL == 2 ? 2 : 1);
     }
     mbar_init(&tmem_full_bar, 1);
-    mbar_init(&tmem_empty_bar, kGemmThreads - 64);
+    mbar_init(&tmem_empty_bar, CL == 4 ? 16 : kGemmThreads - 64);  // pair: one arrival per epilogue warp of both CTAs
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc(&tmem_slot, 512);
+  if (warp == 1) {
+    if (CL == 4) tmem_alloc_pair(&tmem_slot, 512);
+    else tmem_alloc(&tmem_slot, 512);
+  }
   tc_fence_before();
   __syncthreads();
-  if (CL == 2) cluster_sync_all();  // the peer's barriers are initialised before anything arrives on them
+  if (CL != 1) cluster_sync_all();  // the peer's barriers are initialised before anything arrives on them
   tc_fence_after();
   const uint32_t tmem_base = tmem_slot;
 
   const uint32_t a_plane_bytes = kTileM * BK;
-  const uint32_t b_plane_bytes = (uint32_t)p.n_tile * BK;
+  const uint32_t b_plane_bytes = (uint32_t)(CL == 4 ? p.n_tile / 2 : p.n_tile) * BK;
   const uint32_t b_off = (uint32_t)s * a_plane_bytes;
 
   if (warp == 0) {
@@ -191,8 +208,19 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
               continue;
             }
             uint8_t* st = smem + (size_t)stage * p.stage_stride;
-            mbar_expect_tx(&full_bar[stage], tx);
             const int kpos = kc0 + kb * BK;
+            if (CL == 4) {
+              // both CTAs' loads count on the LEADER's full barrier, which expects the bytes of both
+              const uint32_t lead_bar = mapa_shared(smem_u32(&full_bar[stage]), 0u);
+              if (crank == 0) mbar_expect_tx(&full_bar[stage], 2u * tx);
+              for (int t = 0; t < P; ++t)
+                tma_load_3d_pair(st + t * a_plane_bytes, &p.mapA, lead_bar, kpos, tm * kTileM, t);
+              for (int u = 0; u < P; ++u)
+                tma_load_3d_pair(st + b_off + u * b_plane_bytes, &p.mapBh, lead_bar, kpos,
+                                 tn * p.n_tile + (int)crank * (p.n_tile / 2), u);
+              continue;
+            }
+            mbar_expect_tx(&full_bar[stage], tx);
             if (CL == 2) {
               for (int t = 0; t < P; ++t)
                 tma_load_3d_mcast(st + t * a_plane_bytes + crank * (64 * BK), &p.mapA2, &full_bar[stage], kpos,
@@ -214,13 +242,14 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     // so descriptors live in uniform registers.  The (w, t, u) nest is flattened on the host into
     // p.pairs (constant bank): per MMA the loop adds two 16-bit offsets to the descriptor address
     // field -- far fewer issue cycles than the MMA's own 64+ cycles.
-    const uint32_t idesc = make_idesc_i8(kTileM, p.n_tile);
+    const uint32_t idesc = make_idesc_i8(CL == 4 ? 2 * kTileM : kTileM, p.n_tile);
     const uint64_t desc_proto = make_smem_desc(0, BK);
     const uint32_t desc_hi = (uint32_t)(desc_proto >> 32);
     const uint32_t desc_lo0 = (uint32_t)desc_proto;  // LBO field, address 0
     const uint32_t smem_base16 = (smem_u32(smem) & 0x3FFFFu) >> 4;
     const uint32_t stage16 = p.stage_stride >> 4;
     uint32_t it = 0, iter = 0;
+    if (CL != 4 || crank == 0) {  // pair mode: only the leader CTA issues (and waits)
     DFE_WORK_LOOP
     for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
       const int kc0 = zk0 + ch * p.kflush;
@@ -248,26 +277,32 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             for (int kk = 0; kk < nkk; ++kk) {
               const uint32_t lo = lo_base + 2u * kk;  // +32 bytes per K step, in 16-byte units
               const uint32_t later = (kb | kk) ? 1u : 0u;
-#pragma unroll 2
+#pragma unroll 4
               for (int i = pr0; i < pr1; ++i) {
                 const uint2 e = p.pairs[i];
                 const uint64_t adesc = ((uint64_t)desc_hi << 32) | (lo + (e.x & 0xFFFFu));
                 const uint64_t bdesc = ((uint64_t)desc_hi << 32) | (lo + (e.x >> 16));
-                mma_i8_ss(tmem_base + (e.y & 0xFFFFu), adesc, bdesc, idesc, later | (e.y >> 16));
+                if (CL == 4) mma_i8_ss_pair(tmem_base + (e.y & 0xFFFFu), adesc, bdesc, idesc, later | (e.y >> 16));
+                else mma_i8_ss(tmem_base + (e.y & 0xFFFFu), adesc, bdesc, idesc, later | (e.y >> 16));
               }
             }
             // frees the smem stage once these MMAs have read it (in both CTAs of a pair: the peer
             // multicasts into this stage too)
-            if (CL == 2) mma_commit_mcast(&empty_bar[stage], (uint16_t)3);
+            if (CL == 4) mma_commit_pair(&empty_bar[stage], (uint16_t)3);
+            else if (CL == 2) mma_commit_mcast(&empty_bar[stage], (uint16_t)3);
             else mma_commit(&empty_bar[stage]);
           }
           __syncwarp();
         }
-        if (elect_one()) mma_commit(&tmem_full_bar);  // accumulators of this pass are complete
+        if (elect_one()) {  // accumulators of this pass are complete (in both CTAs of a pair)
+          if (CL == 4) mma_commit_pair(&tmem_full_bar, (uint16_t)3);
+          else mma_commit(&tmem_full_bar);
+        }
         __syncwarp();
       }
     }
     }  // work loop
+    }
   } else {
     // ================= epilogue: TMEM -> FP64 recombination -> global =================
     const int quarter = warp & 3;
@@ -429,7 +464,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         }
         if (p.tp && !last) tmem_st_wait();
         tc_fence_before();
-        mbar_arrive(&tmem_empty_bar);
+        if (CL == 4) {  // one arrival per warp on the leader's barrier
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(mapa_shared(smem_u32(&tmem_empty_bar), 0u));
+        } else {
+          mbar_arrive(&tmem_empty_bar);
+        }
       }
     }
     if (p.mode == kEpiX && row_ok) {
@@ -442,10 +482,11 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
 
   tc_fence_before();
   __syncthreads();
-  if (CL == 2) cluster_sync_all();  // no CTA leaves while its peer may still write to it
+  if (CL != 1) cluster_sync_all();  // no CTA leaves while its peer may still write to it
   if (warp == 1) {
     tc_fence_after();
-    tmem_dealloc(tmem_base, 512);
+    if (CL == 4) tmem_dealloc_pair(tmem_base, 512);
+    else tmem_dealloc(tmem_base, 512);
   }
 }
 
@@ -567,14 +608,16 @@ static bool make_plane_map(CUtensorMap* map, const int8_t* base, int64_t k, int6
 }
 
 static uint32_t stage_stride_for(int s, int n_tile, int bk) {
-  return (uint32_t)round_up((int64_t)s * (kTileM + n_tile) * bk, 1024);
+  return (uint32_t)round_up((int64_t)s * (kTileM + n_tile) * bk, 1024);  // n_tile / 2 passed in pair mode
 }
 
 static int g_gemm_dbg_flags = 0;
 static int g_gemm_force_bk = 0;
 static int g_gemm_no_tp = 0;
+static int g_gemm_no_pair = 0;
 void set_gemm_debug_flags(int flags) {
   g_gemm_dbg_flags = flags & 3;
+  g_gemm_no_pair = (flags >> 20) & 1;  // bit 20: no cta_group::2 pair tiles
   g_gemm_no_tp = (flags >> 3) & 1;  // bit 3: multi-pass through global read-modify-write instead of TMEM
   const int f = (flags >> 8) & 0xFF;  // bits 8..15: force the K-block width (32, 64, 128; 0 = auto)
   g_gemm_force_bk = (f == 32 || f == 64 || f == 128) ? f : 0;
@@ -583,18 +626,24 @@ void set_gemm_debug_flags(int flags) {
 cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   GemmKernelParams p;
   const int s = g.s;
+  // cta_group::2 pair: 256-row tiles on an SM pair, each CTA holds half of the B tile's N rows --
+  // the MMA then reads 6 KB instead of 8 KB of shared memory per 128 x 128 x 32 step
+  const bool pair = g.pair && g.n_tile == 128 && g.mode == kEpiC && g.a_rows > kTileM && g_gemm_dbg_flags == 0 &&
+                    !g_gemm_no_pair;
+  const int nb = pair ? g.n_tile / 2 : g.n_tile;  // B rows per CTA and stage
   int bk = g.bk;
   if (bk == 0) bk = g_gemm_force_bk;
   if (bk == 0) {
-    // widest swizzle span that still gives three stages; failing that, two 64-byte stages
-    auto stages = [&](int cand) { return (kSmemLimit - 2048) / (int)stage_stride_for(s, g.n_tile, cand); };
-    if (stages(128) >= 3) bk = 128;
+    // widest swizzle span that still gives two stages (measured: 128-byte K blocks with two stages
+    // beat 64-byte blocks with four: full 128-byte lines per TMA row and half the barrier traffic)
+    auto stages = [&](int cand) { return (kSmemLimit - 2048) / (int)stage_stride_for(s, nb, cand); };
+    if (stages(128) >= 2) bk = 128;
     else if (stages(64) >= 2) bk = 64;
     else bk = 32;
   }
   // a forced K-block width that leaves no room for even one stage is narrowed
-  while (bk > 32 && (kSmemLimit - 2048) / (int)stage_stride_for(s, g.n_tile, bk) < 1) bk /= 2;
-  p.stage_stride = stage_stride_for(s, g.n_tile, bk);
+  while (bk > 32 && (kSmemLimit - 2048) / (int)stage_stride_for(s, nb, bk) < 1) bk /= 2;
+  p.stage_stride = stage_stride_for(s, nb, bk);
   p.num_stages = (int)((kSmemLimit - 2048) / p.stage_stride);
   if (p.num_stages > kMaxStages) p.num_stages = kMaxStages;
   if (p.num_stages < 1) return cudaErrorInvalidValue;
@@ -626,7 +675,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   }
   {
     const int npass = p.npass;
-    const uint32_t a_plane = (uint32_t)kTileM * bk, b_plane = (uint32_t)g.n_tile * bk, b_off = (uint32_t)s * a_plane;
+    const uint32_t a_plane = (uint32_t)kTileM * bk, b_plane = (uint32_t)nb * bk, b_off = (uint32_t)s * a_plane;
     int np = 0;
     for (int ps = 0; ps < npass; ++ps) {
       p.pass_start[ps] = np;
@@ -687,7 +736,14 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.dbg_chunk = g.dbg_chunk;
   p.dbg_flags = g_gemm_dbg_flags;
 
-  p.tiles_per_z = g.lower_only ? p.tiles_m * (p.tiles_m + 1) / 2 : p.tiles_m * p.tiles_n;
+  p.pair = pair ? 1 : 0;
+  const int tiles_m2 = (p.tiles_m + 1) / 2;  // 256-row tiles of the pair mode
+  p.tiles_per_z = pair ? (g.lower_only ? tiles_m2 * (tiles_m2 + 1) : tiles_m2 * p.tiles_n)
+                       : (g.lower_only ? p.tiles_m * (p.tiles_m + 1) / 2 : p.tiles_m * p.tiles_n);
+  if (pair) {
+    p.tiles_m = tiles_m2;  // decode_work rasterises pair rows; the kernel maps them back to 2 tm2 + rank
+    if (!make_plane_map(&p.mapBh, g.B, g.k, g.b_rows, s, g.b_pitch, g.b_plane_stride, bk, 64)) return cudaErrorInvalidValue;
+  }
   p.total_work = (long long)p.tiles_per_z * g.nz;
   static int num_sms = 0;
   if (!num_sms) {
@@ -697,7 +753,8 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   }
   const size_t smem = (size_t)p.num_stages * p.stage_stride + 1024;
   // cluster pair: the two N tiles of an M tile share the A operand through TMA multicast
-  const int cl = (g.cluster_n == 2 && p.tiles_n == 2 && !g.lower_only && g_gemm_dbg_flags == 0 && num_sms >= 2) ? 2 : 1;
+  const int cl = pair ? 4
+                 : (g.cluster_n == 2 && p.tiles_n == 2 && !g.lower_only && g_gemm_dbg_flags == 0 && num_sms >= 2) ? 2 : 1;
   if (cl == 2) {
     p.group_m = 1;  // work items 2c, 2c+1 = (tm = c, tn = 0 / 1)
     if (!make_plane_map(&p.mapA2, g.A, g.k, g.a_rows, s, g.a_pitch, g.a_plane_stride, bk, 64)) return cudaErrorInvalidValue;
@@ -706,9 +763,9 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   // to the hardware scheduler, which balances them better than a static round-robin
   const long long k_item = g.zk ? g.k / (g.nz > 0 ? g.nz : 1) : g.k;
   const bool persistent = cl == 2 || k_item <= 8192;
-  long long nblocks = p.total_work;
+  long long nblocks = cl == 4 ? 2 * p.total_work : p.total_work;  // pair mode: one work item per cluster
   if (persistent && nblocks > num_sms) nblocks = num_sms;
-  if (cl == 2) nblocks = (nblocks + 1) / 2 * 2;
+  if (cl != 1) nblocks = (nblocks + 1) / 2 * 2;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)nblocks, 1, 1);
   cfg.blockDim = dim3(kGemmThreads, 1, 1);
@@ -716,7 +773,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = cl;
+  attr[0].val.clusterDim.x = cl == 1 ? 1 : 2;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
@@ -727,7 +784,9 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   if (err != cudaSuccess) return err;                                                                           \
   err = cudaLaunchKernelEx(&cfg, gemm_i8_kernel<BKV, CLV>, p);                                                  \
   if (err != cudaSuccess) return err;
-  if (cl == 2) {
+  if (cl == 4) {
+    if (bk == 128) { DFE_LAUNCH(128, 4) } else if (bk == 64) { DFE_LAUNCH(64, 4) } else { DFE_LAUNCH(32, 4) }
+  } else if (cl == 2) {
     if (bk == 128) { DFE_LAUNCH(128, 2) } else if (bk == 64) { DFE_LAUNCH(64, 2) } else { DFE_LAUNCH(32, 2) }
   } else {
     if (bk == 128) { DFE_LAUNCH(128, 1) } else if (bk == 64) { DFE_LAUNCH(64, 1) } else { DFE_LAUNCH(32, 1) }

@@ -46,6 +46,7 @@ struct GemmProblem {
   const int32_t* eA;  // scale indices, eA[z * ea_stride + row]
   const int32_t* eB;
   int64_t ea_stride, eb_stride;
+  int pair;           // 1: 256-row tiles on CTA pairs with cta_group::2 MMAs (n_tile 128, FP64 C output)
   int cluster_n;      // 2: CTA pairs over the two N tiles share the A operand by TMA multicast
   int lower_only;     // 1: skip tiles strictly above the block diagonal (GEMM(6))
   int mode;           // EpiMode
