@@ -334,7 +334,16 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     // 12.6 / 15.9 / 20.5 ms at s = 4 / 5 / 6 against 13.8 / 19.8 / 26.8 ms for one 160-column tile
     // in two or more passes -- N = 160 MMAs are shared-memory-bandwidth bound)
     g5.n_tile = w.a_pad;
-    if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) g5.n_tile = w.a_pad / 2;
+    {
+      const int W0 = 512 / (int)round_up(w.a_pad, 32);
+      if (s == W0 + 1 && W0 >= 3 && w.a_pad % 32 == 0 && g_g5_split_n) {
+        // one more weight than TMEM slots: the whole a_pad on cta_group::2 pairs, second pass (one
+        // weight) with the running sum parked in TMEM -- 11.9 vs 12.9 ms at nocc = 150, s = 4
+        g5.pair = 1;
+      } else if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) {
+        g5.n_tile = w.a_pad / 2;
+      }
+    }
     g5.acc_stride = (g5.n_tile % 32) ? g5.n_tile : 0;
     g5.x_cols = w.a_pad;
     g5.cluster_n = (g_g5_cluster && g5.n_tile * 2 == w.a_pad) ? 2 : 1;

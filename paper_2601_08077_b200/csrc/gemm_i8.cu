@@ -628,8 +628,8 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   const int s = g.s;
   // cta_group::2 pair: 256-row tiles on an SM pair, each CTA holds half of the B tile's N rows --
   // the MMA then reads 6 KB instead of 8 KB of shared memory per 128 x 128 x 32 step
-  const bool pair = g.pair && g.n_tile == 128 && g.mode == kEpiC && g.a_rows > kTileM && g_gemm_dbg_flags == 0 &&
-                    !g_gemm_no_pair;
+  const bool pair = g.pair && g.n_tile % 32 == 0 && g.mode != kEpiInt32 && g.a_rows > kTileM &&
+                    (!g.lower_only || g.n_tile == 128) && g_gemm_dbg_flags == 0 && !g_gemm_no_pair;
   const int nb = pair ? g.n_tile / 2 : g.n_tile;  // B rows per CTA and stage
   int bk = g.bk;
   if (bk == 0) bk = g_gemm_force_bk;
@@ -742,7 +742,8 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
                        : (g.lower_only ? p.tiles_m * (p.tiles_m + 1) / 2 : p.tiles_m * p.tiles_n);
   if (pair) {
     p.tiles_m = tiles_m2;  // decode_work rasterises pair rows; the kernel maps them back to 2 tm2 + rank
-    if (!make_plane_map(&p.mapBh, g.B, g.k, g.b_rows, s, g.b_pitch, g.b_plane_stride, bk, 64)) return cudaErrorInvalidValue;
+    if (!make_plane_map(&p.mapBh, g.B, g.k, g.b_rows, s, g.b_pitch, g.b_plane_stride, bk, g.n_tile / 2))
+      return cudaErrorInvalidValue;
   }
   p.total_work = (long long)p.tiles_per_z * g.nz;
   static int num_sms = 0;
