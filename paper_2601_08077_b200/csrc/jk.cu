@@ -50,6 +50,30 @@ struct PackedRowWalker {
   }
 };
 
+// 16 consecutive elements (R, Cs .. Cs+15) of the unpacked matrix for one q (bq = Bp + q).
+// KIND 0: every C < R (consecutive packed rows, constant stride); KIND 1: every C > R (the mirror:
+// packed rows p(C, R), stride growing by one row per column); KIND 2: mixed (diagonal blocks).
+// FULL: all 16 columns are < nao.  The split keeps the address arithmetic at ~2 instructions per
+// element; the generic walker with per-element predicates cost ~17 and made the passes issue bound.
+template <int KIND, bool FULL>
+__device__ __forceinline__ void load_row16(double (&x)[16], const double* __restrict__ bq, int naux, int R, int Cs,
+                                           int nao) {
+  if (KIND == 0) {
+    const double* ptr = bq + ((long long)R * (R + 1) / 2 + Cs) * naux;
+#pragma unroll
+    for (int cc = 0; cc < 16; ++cc) x[cc] = (FULL || Cs + cc < nao) ? __ldg(ptr + (long long)cc * naux) : 0.0;
+  } else if (KIND == 1) {
+    const int row0 = Cs * (Cs + 1) / 2 + R;  // p(Cs, R); p(Cs + cc, R) = row0 + cc Cs + cc (cc + 1) / 2
+#pragma unroll
+    for (int cc = 0; cc < 16; ++cc)
+      x[cc] = (FULL || Cs + cc < nao) ? __ldg(bq + (long long)(row0 + cc * Cs + cc * (cc + 1) / 2) * naux) : 0.0;
+  } else {
+    PackedRowWalker wk(R, Cs);
+#pragma unroll
+    for (int cc = 0; cc < 16; ++cc, wk.next()) x[cc] = (FULL || Cs + cc < nao) ? __ldg(bq + wk.p * naux) : 0.0;
+  }
+}
+
 __device__ __forceinline__ long long packed_row(int R, int C) {
   const long long hi = max(R, C), lo = min(R, C);
   return hi * (hi + 1) / 2 + lo;
@@ -87,16 +111,26 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
     const int R = TR * 32 + rl;
     if (R >= nao) break;
     uint32_t hm = 0;
-    const int c_end = min(32, nao - TC * 32);
-    PackedRowWalker wk(R, TC * 32);
     const double* bq = Bp + (q_ok ? q : 0);
+    const int kind = (TR > TC) ? 0 : (TR < TC) ? 1 : 2;  // block-uniform
+    const bool full = TC * 32 + 32 <= nao;
     // 16 loads in flight per thread before the first use (HBM-latency bound otherwise)
 #pragma unroll
     for (int half = 0; half < 2; ++half) {
       double x[16];
+      const int Cs = TC * 32 + half * 16;
+      if (!q_ok) {
 #pragma unroll
-      for (int cc = 0; cc < 16; ++cc, wk.next())
-        x[cc] = (q_ok && half * 16 + cc < c_end) ? __ldg(bq + wk.p * naux) : 0.0;
+        for (int cc = 0; cc < 16; ++cc) x[cc] = 0.0;
+      } else if (full) {
+        if (kind == 0) load_row16<0, true>(x, bq, naux, R, Cs, nao);
+        else if (kind == 1) load_row16<1, true>(x, bq, naux, R, Cs, nao);
+        else load_row16<2, true>(x, bq, naux, R, Cs, nao);
+      } else {
+        if (kind == 0) load_row16<0, false>(x, bq, naux, R, Cs, nao);
+        else if (kind == 1) load_row16<1, false>(x, bq, naux, R, Cs, nao);
+        else load_row16<2, false>(x, bq, naux, R, Cs, nao);
+      }
 #pragma unroll
       for (int cc = 0; cc < 16; ++cc) {
         hm = max(hm, abs_hi_word(x[cc]));
@@ -165,14 +199,26 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
   const double scale = pow2_double(63 - e);
   const double* bq = Bp + q;
   uint32_t w[S][8];
-  PackedRowWalker wk(R, C0);
+  // block-uniform shape of the tile: rows in block A, columns in block B
+  const int kind = (A > B) ? 0 : (A < B) ? 1 : 2;
+  const bool full = B * 128 + 128 <= nao;
   // all loads of a half are issued before the first conversion (16 requests in flight per thread)
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
     double x[16];
+    const int Cs = C0 + half * 16;
+    if (dbg & 2) {
 #pragma unroll
-    for (int cc = 0; cc < 16; ++cc, wk.next())
-      x[cc] = (C0 + half * 16 + cc < nao && !(dbg & 2)) ? __ldg(bq + wk.p * naux) : 0.0;
+      for (int cc = 0; cc < 16; ++cc) x[cc] = 0.0;
+    } else if (full) {
+      if (kind == 0) load_row16<0, true>(x, bq, naux, R, Cs, nao);
+      else if (kind == 1) load_row16<1, true>(x, bq, naux, R, Cs, nao);
+      else load_row16<2, true>(x, bq, naux, R, Cs, nao);
+    } else {
+      if (kind == 0) load_row16<0, false>(x, bq, naux, R, Cs, nao);
+      else if (kind == 1) load_row16<1, false>(x, bq, naux, R, Cs, nao);
+      else load_row16<2, false>(x, bq, naux, R, Cs, nao);
+    }
 #pragma unroll
     for (int g4 = 0; g4 < 4; ++g4) {
       uint32_t hi[4], lo[4];
