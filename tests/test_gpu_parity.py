@@ -367,3 +367,84 @@ def test_jk_large_config3_sampled(dfe, gpu_ws):
             scale = np.sqrt(np.sum(rows[i] ** 2) * np.sum(rows[j] ** 2))
             assert abs(Kh[i, j] - kij) <= tol * scale, (i, j, Kh[i, j], kij)
     assert np.sum(D * Kh) >= 0.0  # Tr(D K) = 2 |C^T X|^2 (R8)
+
+
+@pytest.mark.parametrize("s", [4, 6])
+def test_jk_nocc_250_like(dfe, gpu_ws, s):
+    """nocc = 250 (config 4's value): a_pad = 256, GEMM(5) runs two N tiles of 128 columns on
+    multicast CTA pairs; s = 6 adds a second pass with the running sum parked in TMEM."""
+    nao, naux, nocc = 264, 12, 250
+    Bp = G.make_B_packed(nao, naux, seed=17)
+    Cocc = G.make_C_occ(nao, nocc, seed=17)
+    D = G.make_density(Cocc)
+    J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+    K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
+    J_ref, K_ref = O.df_jk_plain(Bp, nao, Cocc, D)
+    assert np.array_equal(X[:, :, :nocc], X_emu)
+    assert not X[:, :, nocc:].any()
+    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert O.rel_frobenius(J, J_ref) <= 1e-12
+    assert O.rel_frobenius(K, K_ref) <= (1e-6 if s == 4 else 1e-10)
+    assert np.array_equal(K, K.T)
+    assert dfe.df_last_status() == 0
+
+
+@pytest.mark.parametrize("s", [4, 7])
+def test_emul_gemm_4096_sampled_rows_bitwise(dfe, gpu_ws, s):
+    """Config-1 size 4096^3 in the launch configuration of the big GEMMs (cta_group::2 pair tiles,
+    persistent grid, 128- or 64-byte K blocks).  The oracle emulates sampled rows of A against all of
+    B: those rows of C must match bit for bit; the whole C within the tolerance of s slices."""
+    n = 4096
+    A, B = G.make_gemm_inputs(n, n, n, seed=21)
+    C = torch.empty((n, n), dtype=torch.float64, device=DEV)
+    dfe.df_emul_gemm_slices(dev(A), dev(B), C, n, n, n, s)
+    torch.cuda.synchronize()
+    Cg = C.cpu().numpy()
+    rows = np.array([0, 1, 127, 128, 255, 256, 2047, 2048, 3000, 4095])
+    eB, DB = O.split_operand(np.ascontiguousarray(B.T), s)
+    eA, DA = O.split_operand(A[rows], s)
+    assert np.array_equal(Cg[rows], O.emul_gemm_digits(eA, DA, eB, DB, s))
+    err = O.rel_frobenius(Cg[rows], O.gemm_plain(A[rows], B))
+    assert err <= (1e-6 if s == 4 else 1e-12), err
+    assert dfe.df_last_status() == 0
+
+
+def test_jk_largest_config4_sampled(dfe, gpu_ws):
+    """BASELINE.json config 4 at full size (nao 1800, naux 6000, nocc 250; packed B 78 GB on the
+    device, naux processed in super-blocks of 512-q blocks that fit the workspace).  Sampled K
+    entries against the oracle's definition from the same bytes, symmetry and the trace invariant."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 120 << 30:
+        pytest.skip("needs ~115 GB of free device memory")
+    cfg = G.CONFIGS["largest"]
+    nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc
+    tol = 1e-6
+    s = dfe.df_slices_for_tol(tol)
+    B = G.make_B_packed_torch(nao, naux, cfg.seed, device=DEV)
+    Cocc = G.make_C_occ(nao, nocc, cfg.seed)
+    D = G.make_density(Cocc)
+    big = dfe.Workspace(dfe.df_jk_workspace_bytes_blocks(nao, naux, nocc, s, 2))  # 1024 q per launch
+    try:
+        J = torch.empty((nao, nao), dtype=torch.float64, device=DEV)
+        K = torch.empty_like(J)
+        dfe.df_jk_build(B, nao, naux, dev(Cocc), nocc, dev(D), tol, J, K)
+        torch.cuda.synchronize()
+        assert dfe.df_last_status() == 0
+    finally:
+        big.close()
+        dfe.df_set_workspace(gpu_ws.view)
+    Jh, Kh = J.cpu().numpy(), K.cpu().numpy()
+    assert np.array_equal(Jh, Jh.T) and np.array_equal(Kh, Kh.T)
+    assert np.isfinite(Jh).all() and np.isfinite(Kh).all()
+
+    def x_rows(i):
+        idx = torch.tensor([max(i, j) * (max(i, j) + 1) // 2 + min(i, j) for j in range(nao)], device=DEV)
+        return B.index_select(0, idx).cpu().numpy().T @ Cocc  # (naux, nocc)
+    rows = {i: x_rows(i) for i in (0, 911, 1799)}
+    for i in rows:
+        for j in rows:
+            kij = float(np.sum(rows[i] * rows[j]))
+            scale = np.sqrt(np.sum(rows[i] ** 2) * np.sum(rows[j] ** 2))
+            assert abs(Kh[i, j] - kij) <= tol * scale, (i, j, Kh[i, j], kij)
+    # J needs all of rho (78 GB streamed to the host): its full-size check is the config-3 test
+    assert np.sum(D * Kh) >= 0.0
