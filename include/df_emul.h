@@ -154,8 +154,15 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
                       int s, double* J, double* K,
                       double* X_out, int32_t* e6_out, int* ngroups_out, void* stream);
 
-/* Timing experiments on the GEMM kernel (results are then garbage): bit 0 = issue no
- * MMAs (operand feed only), bit 1 = issue no TMA loads (MMA issue only).  0 = normal. */
+/* Knobs for timing experiments and for forcing the alternative code paths in tests; 0 = the
+ * library's own choices.  Results stay correct except with bits 0, 1, 4, 5.
+ *   bit 0      GEMM issues no MMAs (operand feed only)        bit 1  GEMM issues no TMA loads
+ *   bit 2      GEMM(5) keeps one N tile of a_pad columns      bit 3  multi-pass tiles keep the FP64
+ *                                                                    running sum in global memory
+ *   bit 4 / 5  unpack kernel writes nothing / reads nothing   bit 6  GEMM(5) N halves without the
+ *                                                                    cluster-pair multicast
+ *   bits 8-15  force the K-block width in bytes (32, 64, 128) bits 16-19 MMA probe: operand tiles
+ *   bit 20     no cta_group::2 pair tiles                            walked (2 bits), swizzle (2 bits) */
 int df_debug_set_gemm_flags(int flags);
 
 /* Number of GPU kernels this library has launched in this process. */

@@ -573,9 +573,9 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t 
 int df_debug_set_gemm_flags(int flags) {
   set_gemm_debug_flags(flags);
   g_g5_split_n = (flags & 4) ? 0 : 1;  // bit 2: GEMM(5) keeps one N tile
-  g_g5_cluster = (flags & 64) ? 0 : 1;
-  set_jk_debug_flags((flags >> 4) & 3);
-  set_peak_tiles((flags >> 16) & 15);  // bits 16,17: MMA probe walks 1..4 operand tiles; bits 18,19: swizzle 32/64/128  // bits 4, 5: unpack kernel without stores / without loads  // bit 2: GEMM(5) keeps one N tile (multi-pass read-modify-write)
+  g_g5_cluster = (flags & 64) ? 0 : 1;  // bit 6: GEMM(5) N halves without the multicast pair
+  set_jk_debug_flags((flags >> 4) & 3);  // bits 4, 5: unpack kernel without stores / without loads
+  set_peak_tiles((flags >> 16) & 15);  // bits 16-19: MMA probe operand tiles / swizzle
   return DF_OK;
 }
 

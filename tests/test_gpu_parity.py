@@ -320,6 +320,7 @@ def test_jk_large_config3_sampled(dfe, gpu_ws):
     the device), in bench.py's launch configuration (all 4000 q in one super-block).  The oracle
     computes sampled outputs one by one from the same bytes: rho (all of it, streamed back in
     chunks), sampled J entries, sampled K entries; plus the invariants that hold at any size."""
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 75 << 30:
         pytest.skip("needs ~70 GB of free device memory")
@@ -413,6 +414,7 @@ def test_jk_largest_config4_sampled(dfe, gpu_ws):
     """BASELINE.json config 4 at full size (nao 1800, naux 6000, nocc 250; packed B 78 GB on the
     device, naux processed in super-blocks of 512-q blocks that fit the workspace).  Sampled K
     entries against the oracle's definition from the same bytes, symmetry and the trace invariant."""
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 120 << 30:
         pytest.skip("needs ~115 GB of free device memory")
@@ -448,3 +450,40 @@ def test_jk_largest_config4_sampled(dfe, gpu_ws):
             assert abs(Kh[i, j] - kij) <= tol * scale, (i, j, Kh[i, j], kij)
     # J needs all of rho (78 GB streamed to the host): its full-size check is the config-3 test
     assert np.sum(D * Kh) >= 0.0
+
+
+@pytest.mark.parametrize("flags", [8, 1 << 20, (1 << 20) | 8, 32 << 8, 64 << 8, 128 << 8])
+def test_emul_gemm_alternative_paths_bitwise(dfe, gpu_ws, flags):
+    """The code paths the library does not pick by itself at these sizes (global read-modify-write
+    of multi-pass tiles, one CTA per tile instead of cta_group::2 pairs, every K-block width) must
+    give the same bits as the oracle's emulation."""
+    m, n, k = 300, 260, 1500
+    A, B = G.make_gemm_inputs(m, n, k, seed=31)
+    Ad, Bd = dev(A), dev(B)
+    dfe.lib.df_debug_set_gemm_flags(flags)
+    try:
+        for s in (3, 6, 8):
+            C = torch.empty((m, n), dtype=torch.float64, device=DEV)
+            dfe.df_emul_gemm_slices(Ad, Bd, C, m, n, k, s)
+            torch.cuda.synchronize()
+            assert np.array_equal(C.cpu().numpy(), O.emul_gemm(A, B, s)), f"s={s}"
+    finally:
+        dfe.lib.df_debug_set_gemm_flags(0)
+
+
+@pytest.mark.parametrize("flags", [4, 64, 4 | 8])
+def test_jk_alternative_gemm5_paths(dfe, gpu_ws, flags):
+    """GEMM(5) with one N tile (multi-pass) and with N halves without the multicast pair."""
+    nao, naux, nocc = 168, 38, 150
+    Bp = G.make_B_packed(nao, naux, seed=13)
+    Cocc = G.make_C_occ(nao, nocc, seed=13)
+    D = G.make_density(Cocc)
+    dfe.lib.df_debug_set_gemm_flags(flags)
+    try:
+        for s in (4, 6):
+            J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+            K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
+            assert np.array_equal(X[:, :, :nocc], X_emu), f"s={s}"
+            assert O.rel_frobenius(K, K_emu) <= 1e-14
+    finally:
+        dfe.lib.df_debug_set_gemm_flags(0)
