@@ -187,7 +187,7 @@ constexpr int kQBlock = 512;  // BASELINE.json config 4: "naux blocks of 512"
 
 struct JkWs {
   int* status;
-  double* rho;
+  double *rho, *rho_part;
   uint32_t* emax5;
   double* Jp;
   uint32_t* cmaxC;
@@ -218,6 +218,7 @@ static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s,
   w.pitch6 = plane_pitch(QS * w.a_pad);
   w.status = c.take<int>(64);
   w.rho = c.take<double>(naux);
+  w.rho_part = c.take<double>(jk_rho_part_rows((int)nao) * naux);
   w.emax5 = c.take<uint32_t>(nao * naux);
   w.Jp = c.take<double>(nao * (nao + 1) / 2);
   w.cmaxC = c.take<uint32_t>(w.a_pad);
@@ -277,11 +278,10 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
   if ((x) != cudaSuccess) return DF_ERR_CUDA;
 
   // ---- J: rho (Eq. 3) fused with GEMM(5)'s row maxima, then J (Eq. 4) ----
-  DFE_CK(cudaMemsetAsync(w.rho, 0, sizeof(double) * naux, st));
   DFE_CK(cudaMemsetAsync(w.emax5, 0, sizeof(uint32_t) * nao * naux, st));
   {
     ProfScope ps(kPPassA, st);
-    DFE_CK(launch_jk_pass_a(Bp, (int)nao, (int)naux, D, w.rho, w.emax5, st));
+    DFE_CK(launch_jk_pass_a(Bp, (int)nao, (int)naux, D, w.rho_part, w.rho, w.emax5, st));
   }
   {
     ProfScope ps(kPJGemv, st);

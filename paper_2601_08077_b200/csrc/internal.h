@@ -73,9 +73,11 @@ cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStrea
 
 void set_jk_debug_flags(int flags);  // timing experiments: bit 0 = unpack writes nothing, bit 1 = reads nothing
 // ---- jk.cu ----------------------------------------------------------------
-// pass A over packed B: rho[q] (+=, must be zeroed) and emax[i * naux + q] = upper word of
-// max_j |B^q_ij| (atomicMax, must be zeroed).
-cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho,
+// pass A over packed B: rho[q] (through rho_part[jk_rho_part_rows(nao)][naux], every element of
+// which is written, summed in a fixed order) and emax[i * naux + q] = upper word of max_j |B^q_ij|
+// (atomicMax, must be zeroed).
+int64_t jk_rho_part_rows(int nao);
+cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho_part, double* rho,
                              uint32_t* emax, cudaStream_t st);
 // J_packed[p] = sum_q B[p, q] rho[q]
 cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const double* rho, double* Jp,

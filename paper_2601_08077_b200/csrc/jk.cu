@@ -80,7 +80,8 @@ __device__ __forceinline__ long long packed_row(int R, int C) {
 }
 
 __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict__ Bp, int nao, int naux,
-                                                        const double* __restrict__ D, double* __restrict__ rho,
+                                                        const double* __restrict__ D,
+                                                        double* __restrict__ rho_part,
                                                         uint32_t* __restrict__ emax) {
   int TR, TC;
   bool lower;
@@ -146,8 +147,39 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
       double t = 0.0;
 #pragma unroll
       for (int w = 0; w < 8; ++w) t += rho_sh[w][lane];
-      atomicAdd(&rho[q], t);
+      rho_part[(long long)blockIdx.y * naux + q] = t;  // one lower block per (tile pair, q chunk)
     }
+  }
+}
+
+// rho[q] = sum over tile pairs of rho_part[pair][q] in a fixed order (eight contiguous runs of
+// pairs, one per warp, then the eight run sums in order): bitwise reproducible, unlike atomics.
+__global__ void __launch_bounds__(256) jk_rho_reduce_kernel(const double* __restrict__ rho_part, int npairs,
+                                                            int naux, double* __restrict__ rho) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int q = blockIdx.x * 32 + lane;
+  __shared__ double part[8][32];
+  const int per = (npairs + 7) / 8;
+  const int y0 = warp * per, y1 = min(npairs, y0 + per);
+  double t = 0.0;
+  if (q < naux) {
+    int y = y0;
+    for (; y + 8 <= y1; y += 8) {
+      double v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) v[u] = __ldg(rho_part + (long long)(y + u) * naux + q);
+#pragma unroll
+      for (int u = 0; u < 8; ++u) t += v[u];
+    }
+    for (; y < y1; ++y) t += __ldg(rho_part + (long long)y * naux + q);
+  }
+  part[warp][lane] = t;
+  __syncthreads();
+  if (warp == 0 && q < naux) {
+    double r = 0.0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) r += part[w][lane];
+    rho[q] = r;
   }
 }
 
@@ -329,11 +361,14 @@ static unsigned tile_pairs(int nao) {
   return T * (T + 1) / 2;
 }
 
-cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho, uint32_t* emax,
-                             cudaStream_t st) {
+int64_t jk_rho_part_rows(int nao) { return tile_pairs(nao); }
+
+cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho_part, double* rho,
+                             uint32_t* emax, cudaStream_t st) {
   dim3 grid(2u * (unsigned)((naux + 31) / 32), tile_pairs(nao));
-  jk_pass_a_kernel<<<grid, 256, 0, st>>>(Bp, nao, naux, D, rho, emax);
-  count_launch();
+  jk_pass_a_kernel<<<grid, 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax);
+  jk_rho_reduce_kernel<<<(unsigned)((naux + 31) / 32), 256, 0, st>>>(rho_part, (int)tile_pairs(nao), naux, rho);
+  count_launch(2);
   return cudaGetLastError();
 }
 

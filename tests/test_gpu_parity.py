@@ -338,6 +338,12 @@ def test_jk_large_config3_sampled(dfe, gpu_ws):
         dfe.df_jk_build(B, nao, naux, dev(Cocc), nocc, dev(D), tol, J, K)
         torch.cuda.synchronize()
         assert dfe.df_last_status() == 0
+        # run-to-run reproducibility: every reduction has a fixed order (no floating-point atomics)
+        J2, K2 = torch.full_like(J, np.nan), torch.full_like(K, np.nan)
+        dfe.df_jk_build(B, nao, naux, dev(Cocc), nocc, dev(D), tol, J2, K2)
+        torch.cuda.synchronize()
+        assert torch.equal(J, J2) and torch.equal(K, K2)
+        del J2, K2
     finally:
         big.close()
         dfe.df_set_workspace(gpu_ws.view)
