@@ -102,7 +102,9 @@ int df_emul_gemm(const double* A, const double* B, double* C,
  * C_occ: nao x nocc.  D: nao x nao, read as symmetric (0.5 (D + D^T)).
  * J, K: nao x nao outputs, both triangles written, exactly symmetric.
  * J is plain FP64; K = sum_q X^q X^q^T (no occupation factor,
- * PAPER.md:53) is emulated with s = df_slices_for_tol(tol) in both GEMMs. */
+ * PAPER.md:53) is emulated with s = df_slices_for_tol(tol) in both GEMMs.
+ * Every reduction has a fixed order: the same inputs and s give the same bits
+ * on every call, whatever the workspace size. */
 int df_jk_build(const double* B_packed, int64_t nao, int64_t naux,
                 const double* C_occ, int64_t nocc, const double* D,
                 double tol, double* J, double* K, void* stream);

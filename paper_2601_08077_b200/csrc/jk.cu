@@ -218,8 +218,10 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int R = A * 128 + (sub & 63) * 2 + (warp >> 2);
   const int q = q0 + (blockIdx.x >> 7) * 32 + (warp & 3) * 8 + (lane >> 2);
-  const int C0 = B * 128 + (lane & 3) * 32;
-  if (R >= nao || q >= q1 || C0 >= pitch) return;
+  // a thread owns columns [C0, C0 + 16) and [C0 + 64, C0 + 80): the four lanes of a q write 64
+  // contiguous bytes per store instruction (whole sectors); pitch is a multiple of 128
+  const int C0 = B * 128 + (lane & 3) * 16;
+  if (R >= nao || q >= q1) return;
   const uint32_t hm = emax[(long long)R * naux + q];
   const int e = scale_index_from_hi(hm);
   const long long orow = (long long)(q - q0) * nao + R;
@@ -238,7 +240,7 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
     double x[16];
-    const int Cs = C0 + half * 16;
+    const int Cs = C0 + half * 64;
     if (dbg & 2) {
 #pragma unroll
       for (int cc = 0; cc < 16; ++cc) x[cc] = 0.0;
@@ -271,7 +273,7 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
     uint4* dst = reinterpret_cast<uint4*>(planes + t * plane_stride + orow * pitch + C0);
     if ((dbg & 1) && w[t][0] != 0x12345678u) continue;
     dst[0] = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
-    dst[1] = make_uint4(w[t][4], w[t][5], w[t][6], w[t][7]);
+    dst[4] = make_uint4(w[t][4], w[t][5], w[t][6], w[t][7]);
   }
 }
 
@@ -395,6 +397,7 @@ cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, 
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
                                    int* status, cudaStream_t st) {
   const unsigned T128 = (unsigned)((nao + 127) / 128);
+  if (pitch % 128 != 0 || pitch < 128 * (int64_t)T128) return cudaErrorInvalidValue;
   dim3 grid(128u * (unsigned)((q1 - q0 + 31) / 32), T128 * (T128 + 1) / 2);
   DFE_DISPATCH_S(s, (jk_unpack_split_kernel<SS><<<grid, 256, 0, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5,
                                                                       pitch, plane_stride, status, g_jk_dbg)));
