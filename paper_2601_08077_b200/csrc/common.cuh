@@ -64,6 +64,17 @@ __device__ __forceinline__ uint32_t pack4_digit(uint32_t h0, uint32_t h1, uint32
   return __byte_perm(__byte_perm(h0, h1, sel), __byte_perm(h2, h3, sel), 0x5410);
 }
 
+// out[b] = byte b of h[0], h[1], h[2], h[3] (a 4 x 4 byte transpose): eight byte permutes for the
+// four plane words of four consecutive elements.
+__device__ __forceinline__ void transpose4x4_bytes(const uint32_t (&h)[4], uint32_t (&out)[4]) {
+  const uint32_t a01 = __byte_perm(h[0], h[1], 0x5140), b01 = __byte_perm(h[0], h[1], 0x7362);
+  const uint32_t a23 = __byte_perm(h[2], h[3], 0x5140), b23 = __byte_perm(h[2], h[3], 0x7362);
+  out[0] = __byte_perm(a01, a23, 0x5410);
+  out[1] = __byte_perm(a01, a23, 0x7632);
+  out[2] = __byte_perm(b01, b23, 0x5410);
+  out[3] = __byte_perm(b01, b23, 0x7632);
+}
+
 __device__ __forceinline__ uint32_t abs_hi_word(double x) {
   return (uint32_t)__double2hiint(x) & 0x7FFFFFFFu;
 }

@@ -35,42 +35,29 @@ __device__ __forceinline__ bool tile_of_block(unsigned idx, int flip, int& TR, i
   return true;
 }
 
-// Walks the packed rows p(R, C) for C = C0, C0+1, ...: consecutive rows while C <= R, then a
-// stride of C+1 rows (p(C, R) = C(C+1)/2 + R).
-struct PackedRowWalker {
-  long long p;
-  int R, C;
-  __device__ __forceinline__ PackedRowWalker(int R_, int C0) : R(R_), C(C0) {
-    const long long hi = max(R_, C0), lo = min(R_, C0);
-    p = hi * (hi + 1) / 2 + lo;
-  }
-  __device__ __forceinline__ void next() {
-    p += (C < R) ? 1 : (C + 1);
-    ++C;
-  }
-};
-
-// 16 consecutive elements (R, Cs .. Cs+15) of the unpacked matrix for one q (bq = Bp + q).
-// KIND 0: every C < R (consecutive packed rows, constant stride); KIND 1: every C > R (the mirror:
-// packed rows p(C, R), stride growing by one row per column); KIND 2: mixed (diagonal blocks).
-// FULL: all 16 columns are < nao.  The split keeps the address arithmetic at ~2 instructions per
-// element; the generic walker with per-element predicates cost ~17 and made the passes issue bound.
+// 16 consecutive elements (R, Cs .. Cs+15) of the unpacked matrix for one q (bqb = byte address of
+// Bp + q, naux8 = bytes per packed row).  KIND 0: every C < R (consecutive packed rows); KIND 1:
+// every C > R (the mirror: packed rows p(C, R), stride growing by one row per column); KIND 2: mixed
+// (diagonal blocks).  FULL: all 16 columns are < nao; otherwise the column is clamped to nao - 1
+// (a valid address) and the value replaced by zero.  Row indices are unsigned 32-bit and the byte
+// offset one 32 x 32 -> 64 multiply-add, 2-3 instructions per element (signed 64-bit index
+// arithmetic cost 5-10 and made the passes issue bound).
 template <int KIND, bool FULL>
-__device__ __forceinline__ void load_row16(double (&x)[16], const double* __restrict__ bq, int naux, int R, int Cs,
-                                           int nao) {
-  if (KIND == 0) {
-    const double* ptr = bq + ((long long)R * (R + 1) / 2 + Cs) * naux;
+__device__ __forceinline__ void load_row16(double (&x)[16], const char* __restrict__ bqb, unsigned naux8, int R,
+                                           int Cs, int nao) {
+  const unsigned uR = (unsigned)R;
 #pragma unroll
-    for (int cc = 0; cc < 16; ++cc) x[cc] = (FULL || Cs + cc < nao) ? __ldg(ptr + (long long)cc * naux) : 0.0;
-  } else if (KIND == 1) {
-    const int row0 = Cs * (Cs + 1) / 2 + R;  // p(Cs, R); p(Cs + cc, R) = row0 + cc Cs + cc (cc + 1) / 2
+  for (int cc = 0; cc < 16; ++cc) {
+    const unsigned c = FULL ? (unsigned)(Cs + cc) : (unsigned)min(Cs + cc, nao - 1);
+    unsigned row;
+    if (KIND == 0) row = uR * (uR + 1) / 2 + c;
+    else if (KIND == 1) row = c * (c + 1) / 2 + uR;
+    else row = (c <= uR) ? uR * (uR + 1) / 2 + c : c * (c + 1) / 2 + uR;
+    x[cc] = __ldg(reinterpret_cast<const double*>(bqb + (unsigned long long)row * naux8));
+  }
+  if (!FULL) {
 #pragma unroll
-    for (int cc = 0; cc < 16; ++cc)
-      x[cc] = (FULL || Cs + cc < nao) ? __ldg(bq + (long long)(row0 + cc * Cs + cc * (cc + 1) / 2) * naux) : 0.0;
-  } else {
-    PackedRowWalker wk(R, Cs);
-#pragma unroll
-    for (int cc = 0; cc < 16; ++cc, wk.next()) x[cc] = (FULL || Cs + cc < nao) ? __ldg(bq + wk.p * naux) : 0.0;
+    for (int cc = 0; cc < 16; ++cc) x[cc] = (Cs + cc < nao) ? x[cc] : 0.0;
   }
 }
 
@@ -112,7 +99,8 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
     const int R = TR * 32 + rl;
     if (R >= nao) break;
     uint32_t hm = 0;
-    const double* bq = Bp + (q_ok ? q : 0);
+    const char* bq = reinterpret_cast<const char*>(Bp + (q_ok ? q : 0));
+    const unsigned naux8 = (unsigned)naux * 8u;
     const int kind = (TR > TC) ? 0 : (TR < TC) ? 1 : 2;  // block-uniform
     const bool full = TC * 32 + 32 <= nao;
     // 16 loads in flight per thread before the first use (HBM-latency bound otherwise)
@@ -124,13 +112,13 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
 #pragma unroll
         for (int cc = 0; cc < 16; ++cc) x[cc] = 0.0;
       } else if (full) {
-        if (kind == 0) load_row16<0, true>(x, bq, naux, R, Cs, nao);
-        else if (kind == 1) load_row16<1, true>(x, bq, naux, R, Cs, nao);
-        else load_row16<2, true>(x, bq, naux, R, Cs, nao);
+        if (kind == 0) load_row16<0, true>(x, bq, naux8, R, Cs, nao);
+        else if (kind == 1) load_row16<1, true>(x, bq, naux8, R, Cs, nao);
+        else load_row16<2, true>(x, bq, naux8, R, Cs, nao);
       } else {
-        if (kind == 0) load_row16<0, false>(x, bq, naux, R, Cs, nao);
-        else if (kind == 1) load_row16<1, false>(x, bq, naux, R, Cs, nao);
-        else load_row16<2, false>(x, bq, naux, R, Cs, nao);
+        if (kind == 0) load_row16<0, false>(x, bq, naux8, R, Cs, nao);
+        else if (kind == 1) load_row16<1, false>(x, bq, naux8, R, Cs, nao);
+        else load_row16<2, false>(x, bq, naux8, R, Cs, nao);
       }
 #pragma unroll
       for (int cc = 0; cc < 16; ++cc) {
@@ -231,12 +219,16 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
     if (stt) atomicOr(status, stt);
   }
   const double scale = pow2_double(63 - e);
-  const double* bq = Bp + q;
-  uint32_t w[S][8];
+  const char* bq = reinterpret_cast<const char*>(Bp + q);
+  const unsigned naux8 = (unsigned)naux * 8u;
   // block-uniform shape of the tile: rows in block A, columns in block B
   const int kind = (A > B) ? 0 : (A < B) ? 1 : 2;
   const bool full = B * 128 + 128 <= nao;
-  // all loads of a half are issued before the first conversion (16 requests in flight per thread)
+  int8_t* const orow_ptr = planes + orow * pitch + C0;
+  // all 16 loads of a half are issued before the first conversion; everything is stored at the end
+  // (storing each half before loading the next one, at 4 blocks per SM, ran 35 % slower: 15.6 ms
+  // against 11.5 ms although loads alone and stores alone were both faster)
+  uint32_t w[S][8];
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
     double x[16];
@@ -245,33 +237,32 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
 #pragma unroll
       for (int cc = 0; cc < 16; ++cc) x[cc] = 0.0;
     } else if (full) {
-      if (kind == 0) load_row16<0, true>(x, bq, naux, R, Cs, nao);
-      else if (kind == 1) load_row16<1, true>(x, bq, naux, R, Cs, nao);
-      else load_row16<2, true>(x, bq, naux, R, Cs, nao);
+      if (kind == 0) load_row16<0, true>(x, bq, naux8, R, Cs, nao);
+      else if (kind == 1) load_row16<1, true>(x, bq, naux8, R, Cs, nao);
+      else load_row16<2, true>(x, bq, naux8, R, Cs, nao);
     } else {
-      if (kind == 0) load_row16<0, false>(x, bq, naux, R, Cs, nao);
-      else if (kind == 1) load_row16<1, false>(x, bq, naux, R, Cs, nao);
-      else load_row16<2, false>(x, bq, naux, R, Cs, nao);
+      if (kind == 1) load_row16<1, false>(x, bq, naux8, R, Cs, nao);
+      else load_row16<2, false>(x, bq, naux8, R, Cs, nao);  // kind 0 has B < A: always full
     }
 #pragma unroll
     for (int g4 = 0; g4 < 4; ++g4) {
-      uint32_t hi[4], lo[4];
+      uint32_t hi[4], lo[4], ph[4], pl[4];
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const uint64_t dg = balanced_digits(x[4 * g4 + j], scale);
         hi[j] = (uint32_t)(dg >> 32);
         lo[j] = (uint32_t)dg;
       }
+      transpose4x4_bytes(hi, ph);
+      if (S > 4) transpose4x4_bytes(lo, pl);
 #pragma unroll
-      for (int t = 0; t < S; ++t)
-        w[t][half * 4 + g4] = (t < 4) ? pack4_digit(hi[0], hi[1], hi[2], hi[3], 3 - t)
-                                      : pack4_digit(lo[0], lo[1], lo[2], lo[3], 7 - t);
+      for (int t = 0; t < S; ++t) w[t][half * 4 + g4] = (t < 4) ? ph[3 - t] : pl[7 - t];
     }
   }
 #pragma unroll
   for (int t = 0; t < S; ++t) {
-    uint4* dst = reinterpret_cast<uint4*>(planes + t * plane_stride + orow * pitch + C0);
     if ((dbg & 1) && w[t][0] != 0x12345678u) continue;
+    uint4* dst = reinterpret_cast<uint4*>(orow_ptr + t * plane_stride);
     dst[0] = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
     dst[4] = make_uint4(w[t][4], w[t][5], w[t][6], w[t][7]);
   }
