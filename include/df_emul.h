@@ -109,6 +109,36 @@ int df_jk_build(const double* B_packed, int64_t nao, int64_t naux,
                 const double* C_occ, int64_t nocc, const double* D,
                 double tol, double* J, double* K, void* stream);
 
+/* ---- plan: B split once for a whole SCF --- */
+
+/* B is computed once and is constant over the SCF; its row scales
+ * and INT8 digit planes do not depend on C_occ, D or tol, and the planes have the
+ * prefix property (R3: a build with s slices reads the first s of smax
+ * planes).  A plan is a caller-owned device buffer (256-byte aligned) of
+ * df_jk_plan_bytes() bytes holding them: naux x nao x (8 + round_up(nao,128) x smax)
+ * bytes, 37 GB at config 3 with smax = 6.  df_jk_plan_create() fills it (row maxima
+ * + unpack + split of all q, the H2 row of SURVEY.md section 8(a)); it needs a
+ * registered workspace only for the status word.  DF_ERR_WORKSPACE if plan_bytes is
+ * too small. */
+int64_t df_jk_plan_bytes(int64_t nao, int64_t naux, int smax);
+int df_jk_plan_create(const double* B_packed, int64_t nao, int64_t naux, int smax,
+                      void* plan, int64_t plan_bytes, void* stream);
+
+/* Workspace of a planned build (no GEMM(5) operand planes in it), nblocks as in
+ * df_jk_workspace_bytes_blocks. */
+int64_t df_jk_planned_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, int s, int64_t nblocks);
+
+/* df_jk_build with GEMM(5)'s left operand read from `plan` (created from the same
+ * B_packed, nao, naux with `smax` planes; the library cannot check that).  B_packed
+ * is still read for rho and J (plain FP64).  Bit-identical to
+ * df_jk_build.  DF_ERR_TOL if the slice count exceeds smax. */
+int df_jk_build_planned(const void* plan, int smax, const double* B_packed, int64_t nao, int64_t naux,
+                        const double* C_occ, int64_t nocc, const double* D,
+                        double tol, double* J, double* K, void* stream);
+int df_jk_build_planned_slices(const void* plan, int smax, const double* B_packed, int64_t nao, int64_t naux,
+                               const double* C_occ, int64_t nocc, const double* D,
+                               int s, double* J, double* K, void* stream);
+
 /* Same two calls with a forced slice count s in 1..8 (config 1's sweep). */
 int df_emul_gemm_slices(const double* A, const double* B, double* C,
                         int64_t m, int64_t n, int64_t k, int s, void* stream);

@@ -50,6 +50,11 @@ _SIG = {
     "df_emul_gemm_slices": (_i32, [_vp, _vp, _vp, _i64, _i64, _i64, _i32, _vp]),
     "df_jk_build": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _f64, _vp, _vp, _vp]),
     "df_jk_build_slices": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
+    "df_jk_plan_bytes": (_i64, [_i64, _i64, _i32]),
+    "df_jk_plan_create": (_i32, [_vp, _i64, _i64, _i32, _vp, _i64, _vp]),
+    "df_jk_planned_workspace_bytes": (_i64, [_i64, _i64, _i64, _i32, _i64]),
+    "df_jk_build_planned": (_i32, [_vp, _i32, _vp, _i64, _i64, _vp, _i64, _vp, _f64, _vp, _vp, _vp]),
+    "df_jk_build_planned_slices": (_i32, [_vp, _i32, _vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
     "df_last_status": (_i32, [_vp, C.POINTER(C.c_int)]),
     "df_debug_split_rows": (_i32, [_vp, _i64, _i64, _i32, _vp, _vp, _vp]),
     "df_debug_split_cols": (_i32, [_vp, _i64, _i64, _i32, _vp, _vp, _vp]),
@@ -181,6 +186,51 @@ def df_jk_build_slices(B_packed, nao, naux, C_occ, nocc, D, s, J, K, stream=None
     f = torch.float64
     _check(lib.df_jk_build_slices(_ptr(B_packed, f), nao, naux, _ptr(C_occ, f), nocc, _ptr(D, f), int(s),
                                   _ptr(J, f), _ptr(K, f), _stream(stream)), "df_jk_build_slices")
+
+
+# ---- plan: B split once for a whole SCF ---------------------------------------------------
+def df_jk_plan_bytes(nao: int, naux: int, smax: int) -> int:
+    return _check(lib.df_jk_plan_bytes(nao, naux, int(smax)), "df_jk_plan_bytes")
+
+
+def df_jk_planned_workspace_bytes(nao: int, naux: int, nocc: int, s: int, nblocks: int) -> int:
+    return _check(lib.df_jk_planned_workspace_bytes(nao, naux, nocc, s, nblocks), "df_jk_planned_workspace_bytes")
+
+
+class Plan:
+    """Owns the device buffer of a plan and fills it from B_packed (a workspace must be registered)."""
+
+    def __init__(self, B_packed, nao: int, naux: int, smax: int, stream=None):
+        import torch
+
+        self.nao, self.naux, self.smax = int(nao), int(naux), int(smax)
+        nbytes = df_jk_plan_bytes(nao, naux, smax)
+        self.buf = torch.empty(nbytes + 256, dtype=torch.uint8, device=B_packed.device)
+        off = (-self.buf.data_ptr()) % 256
+        self.view = self.buf[off: off + nbytes]
+        _check(lib.df_jk_plan_create(_ptr(B_packed, torch.float64), nao, naux, int(smax), _ptr(self.view), nbytes,
+                                     _stream(stream)), "df_jk_plan_create")
+
+    def close(self):
+        self.buf = self.view = None
+
+
+def df_jk_build_planned(plan, B_packed, nao, naux, C_occ, nocc, D, tol, J, K, stream=None) -> None:
+    import torch
+
+    f = torch.float64
+    _check(lib.df_jk_build_planned(_ptr(plan.view), plan.smax, _ptr(B_packed, f), nao, naux, _ptr(C_occ, f), nocc,
+                                   _ptr(D, f), float(tol), _ptr(J, f), _ptr(K, f), _stream(stream)),
+           "df_jk_build_planned")
+
+
+def df_jk_build_planned_slices(plan, B_packed, nao, naux, C_occ, nocc, D, s, J, K, stream=None) -> None:
+    import torch
+
+    f = torch.float64
+    _check(lib.df_jk_build_planned_slices(_ptr(plan.view), plan.smax, _ptr(B_packed, f), nao, naux, _ptr(C_occ, f),
+                                          nocc, _ptr(D, f), int(s), _ptr(J, f), _ptr(K, f), _stream(stream)),
+           "df_jk_build_planned_slices")
 
 
 def df_last_status(stream=None) -> int:

@@ -205,8 +205,28 @@ struct JkWs {
   int a_pad, QG, gpb, ngmax;
 };
 
-// QS = q per super-block (a multiple of 512, or naux when naux < 512)
-static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s, int64_t QS) {
+// Plan buffer (df_jk_plan_create): everything about B that does not change over an SCF.
+//   [emax5: nao x naux u32][e5: (q, i) i32][planes: smax x (q, i) x pitch int8]
+// The digit planes have the prefix property (R3): a build with s <= smax slices reads
+// the first s planes.
+struct PlanLayout {
+  int64_t pitch, rows, emax_off, e5_off, planes_off, plane_stride, bytes;
+};
+static PlanLayout plan_layout(int64_t nao, int64_t naux, int smax) {
+  PlanLayout L;
+  L.pitch = round_up(nao, 128);
+  L.rows = naux * nao;
+  L.emax_off = 0;
+  L.e5_off = round_up(L.rows * 4, 256);
+  L.planes_off = L.e5_off + round_up(L.rows * 4, 256);
+  L.plane_stride = L.rows * L.pitch;
+  L.bytes = L.planes_off + smax * L.plane_stride;
+  return L;
+}
+
+// QS = q per super-block (a multiple of 512, or naux when naux < 512); planned: GEMM(5)'s left
+// operand comes from a plan, no emax5 / e5 / planes5 in the workspace
+static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s, int64_t QS, bool planned = false) {
   Carver c(base);
   JkWs w;
   w.a_pad = pad16(nocc);
@@ -220,13 +240,13 @@ static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s,
   w.status = c.take<int>(64);
   w.rho = c.take<double>(naux);
   w.rho_part = c.take<double>(jk_rho_part_rows((int)nao) * naux);
-  w.emax5 = c.take<uint32_t>(nao * naux);
+  w.emax5 = planned ? nullptr : c.take<uint32_t>(nao * naux);
   w.Jp = c.take<double>(nao * (nao + 1) / 2);
   w.cmaxC = c.take<uint32_t>(w.a_pad);
   w.eC = c.take<int32_t>(w.a_pad);
   w.pc = c.take<int8_t>((int64_t)s * w.a_pad * w.pitchj);
-  w.e5 = c.take<int32_t>(QS * nao);
-  w.p5 = c.take<int8_t>((int64_t)s * QS * nao * w.pitchj);
+  w.e5 = planned ? nullptr : c.take<int32_t>(QS * nao);
+  w.p5 = planned ? nullptr : c.take<int8_t>((int64_t)s * QS * nao * w.pitchj);
   w.X = c.take<double>(nao * QS * w.a_pad);
   w.qgroup = c.take<int>(QS);
   w.gcol = c.take<int>(w.ngmax + 1);
@@ -249,10 +269,14 @@ __global__ void jk_group_tables_kernel(int nq, int QG, int gpb, int a_pad, int n
   }
 }
 
+// plan != nullptr (with its slice count smax): a planned build, GEMM(5) reads the plan's planes.
 static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Cocc, int64_t nocc, const double* D,
                    int s, double* J, double* K, double* X_out, int32_t* e6_out, int* ngroups_out,
-                   cudaStream_t st) {
+                   cudaStream_t st, const void* plan = nullptr, int smax = 0) {
   if (!Bp || !Cocc || !D || !J || !K) return DF_ERR_NULL;
+  const bool planned = plan != nullptr;
+  if (planned && (smax < 1 || smax > kMaxSlices || s > smax)) return DF_ERR_TOL;
+  if (planned && ((uintptr_t)plan & 255) != 0) return DF_ERR_ALIGN;
   if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nao > 11552 || naux > (1 << 20)) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
   if (!device_ok()) return DF_ERR_DEVICE;
@@ -265,21 +289,23 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     for (int64_t nb = nblk; nb >= 1; --nb) {
       const int64_t qs = (nb == nblk) ? naux : nb * kQBlock;
       if (qs * pad16(nocc) >= (1ll << 30) || qs * nao >= (1ll << 31) - 256) continue;
-      if (carve_jk(nullptr, nao, naux, nocc, s, qs).bytes <= g_ws_bytes) {
+      if (carve_jk(nullptr, nao, naux, nocc, s, qs, planned).bytes <= g_ws_bytes) {
         QS = qs;
         break;
       }
     }
   }
   if (QS == 0) return DF_ERR_WORKSPACE;
-  JkWs w = carve_jk(g_ws, nao, naux, nocc, s, QS);
+  JkWs w = carve_jk(g_ws, nao, naux, nocc, s, QS, planned);
+  const PlanLayout PL = plan_layout(nao, naux, planned ? smax : 1);
+  const char* const plan_b = static_cast<const char*>(plan);
   const int64_t npair = nao * (nao + 1) / 2;
 
 #define DFE_CK(x) \
   if ((x) != cudaSuccess) return DF_ERR_CUDA;
 
   // ---- J: rho (Eq. 3) fused with GEMM(5)'s row maxima, then J (Eq. 4) ----
-  DFE_CK(cudaMemsetAsync(w.emax5, 0, sizeof(uint32_t) * nao * naux, st));
+  if (!planned) DFE_CK(cudaMemsetAsync(w.emax5, 0, sizeof(uint32_t) * nao * naux, st));
   {
     ProfScope ps(kPPassA, st);
     DFE_CK(launch_jk_pass_a(Bp, (int)nao, (int)naux, D, w.rho_part, w.rho, w.emax5, st));
@@ -313,21 +339,21 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     DFE_CK(cudaGetLastError());
     DFE_CK(cudaMemsetAsync(w.xmax, 0, sizeof(uint32_t) * ng * nao, st));
 
-    // H2: unpack + split packed B -> planes5 rows (q, i), contraction j
-    {
+    // H2: unpack + split packed B -> planes5 rows (q, i), contraction j (a plan holds them already)
+    if (!planned) {
       ProfScope ps(kPUnpack, st);
       DFE_CK(launch_jk_unpack_split(Bp, (int)nao, (int)naux, (int)qs0, (int)qs1, w.emax5, s, w.e5, w.p5,
                                     w.pitchj, (int64_t)nq * nao * w.pitchj, w.status, st));
     }
     // GEMM(5): X[i][q][a] = sum_j B^q_ij C_ja   (Eq. 5 / Eq. 12)
     GemmProblem g5 = {};
-    g5.A = w.p5;
+    g5.A = planned ? reinterpret_cast<const int8_t*>(plan_b + PL.planes_off) + qs0 * nao * PL.pitch : w.p5;
     g5.B = w.pc;
     g5.a_rows = (int64_t)nq * nao;
     g5.b_rows = w.a_pad;
     g5.k = nao;
     g5.a_pitch = g5.b_pitch = w.pitchj;
-    g5.a_plane_stride = (int64_t)nq * nao * w.pitchj;
+    g5.a_plane_stride = planned ? PL.plane_stride : (int64_t)nq * nao * w.pitchj;
     g5.b_plane_stride = (int64_t)w.a_pad * w.pitchj;
     g5.s = s;
     // N tile: the whole a_pad when all s weight accumulators fit TMEM (s * a_pad <= 512 columns), else
@@ -349,7 +375,7 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     g5.x_cols = w.a_pad;
     g5.cluster_n = (g_g5_cluster && g5.n_tile * 2 == w.a_pad) ? 2 : 1;
     g5.nz = 1;
-    g5.eA = w.e5;
+    g5.eA = planned ? reinterpret_cast<const int32_t*>(plan_b + PL.e5_off) + qs0 * nao : w.e5;
     g5.eB = w.eC;
     g5.mode = kEpiX;
     g5.C = w.X;
@@ -496,6 +522,68 @@ int df_jk_build(const double* B_packed, int64_t nao, int64_t naux, const double*
 int df_jk_build_slices(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
                        const double* D, int s, double* J, double* K, void* stream) {
   return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+int64_t df_jk_plan_bytes(int64_t nao, int64_t naux, int smax) {
+  if (nao <= 0 || naux <= 0 || nao > 11552 || naux > (1 << 20)) return DF_ERR_DIM;
+  if (smax < 1 || smax > kMaxSlices) return DF_ERR_TOL;
+  return plan_layout(nao, naux, smax).bytes;
+}
+
+int df_jk_plan_create(const double* B_packed, int64_t nao, int64_t naux, int smax, void* plan, int64_t plan_bytes,
+                      void* stream) {
+  if (!B_packed || !plan) return DF_ERR_NULL;
+  if (nao <= 0 || naux <= 0 || nao > 11552 || naux > (1 << 20)) return DF_ERR_DIM;
+  if (smax < 1 || smax > kMaxSlices) return DF_ERR_TOL;
+  if (((uintptr_t)plan & 255) != 0) return DF_ERR_ALIGN;
+  if (!device_ok()) return DF_ERR_DEVICE;
+  if (!g_ws) return DF_ERR_WORKSPACE;  // the status word
+  const PlanLayout L = plan_layout(nao, naux, smax);
+  if (plan_bytes < L.bytes) return DF_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  char* pb = static_cast<char*>(plan);
+  uint32_t* emax = reinterpret_cast<uint32_t*>(pb + L.emax_off);
+  if (cudaMemsetAsync(emax, 0, sizeof(uint32_t) * L.rows, st) != cudaSuccess) return DF_ERR_CUDA;
+  {
+    ProfScope ps(kPPassA, st);
+    if (launch_jk_pass_a(B_packed, (int)nao, (int)naux, nullptr, nullptr, nullptr, emax, st) != cudaSuccess)
+      return DF_ERR_CUDA;
+  }
+  {
+    ProfScope ps(kPUnpack, st);
+    if (launch_jk_unpack_split(B_packed, (int)nao, (int)naux, 0, (int)naux, emax, smax,
+                               reinterpret_cast<int32_t*>(pb + L.e5_off),
+                               reinterpret_cast<int8_t*>(pb + L.planes_off), L.pitch, L.plane_stride,
+                               (int*)g_ws, st) != cudaSuccess)
+      return DF_ERR_CUDA;
+  }
+  return DF_OK;
+}
+
+int64_t df_jk_planned_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, int s, int64_t nblocks) {
+  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nblocks < 1) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  int64_t qs = nblocks * kQBlock;
+  if (qs > naux) qs = naux;
+  return carve_jk(nullptr, nao, naux, nocc, s, qs, true).bytes;
+}
+
+int df_jk_build_planned(const void* plan, int smax, const double* B_packed, int64_t nao, int64_t naux,
+                        const double* C_occ, int64_t nocc, const double* D, double tol, double* J, double* K,
+                        void* stream) {
+  if (!plan) return DF_ERR_NULL;
+  const int s = slices_for_tol(tol, g_mode);
+  if (s < 0) return s;
+  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream,
+                 plan, smax);
+}
+
+int df_jk_build_planned_slices(const void* plan, int smax, const double* B_packed, int64_t nao, int64_t naux,
+                               const double* C_occ, int64_t nocc, const double* D, int s, double* J, double* K,
+                               void* stream) {
+  if (!plan) return DF_ERR_NULL;
+  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream,
+                 plan, smax);
 }
 
 int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,

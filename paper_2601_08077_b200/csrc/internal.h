@@ -75,7 +75,8 @@ void set_jk_debug_flags(int flags);  // timing experiments: bit 0 = unpack write
 // ---- jk.cu ----------------------------------------------------------------
 // pass A over packed B: rho[q] (through rho_part[jk_rho_part_rows(nao)][naux], every element of
 // which is written, summed in a fixed order) and emax[i * naux + q] = upper word of max_j |B^q_ij|
-// (atomicMax, must be zeroed).
+// (atomicMax, must be zeroed).  rho == nullptr: the maxima alone (df_jk_plan_create); emax == nullptr:
+// rho alone, lower tiles only (planned builds).
 int64_t jk_rho_part_rows(int nao);
 cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho_part, double* rho,
                              uint32_t* emax, cudaStream_t st);

@@ -66,6 +66,9 @@ __device__ __forceinline__ long long packed_row(int R, int C) {
   return hi * (hi + 1) / 2 + lo;
 }
 
+// RHO: the rho partials (lower tiles only); EMAX: the row maxima (lower tiles and their mirrors).
+// A plan (df_jk_plan_create) runs EMAX alone once, a planned build RHO alone (half the blocks).
+template <bool RHO, bool EMAX>
 __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict__ Bp, int nao, int naux,
                                                         const double* __restrict__ D,
                                                         double* __restrict__ rho_part,
@@ -74,13 +77,15 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
   bool lower;
   // blockIdx.x = 2 * q-chunk + flip: a tile and its mirror read the same 256 KB back to back (the
   // second read is an L2 hit) and neighbouring blocks read adjacent 256-byte runs of the same rows
-  if (!tile_of_block(blockIdx.y, blockIdx.x & 1, TR, TC, lower)) return;
+  const int flip = EMAX ? (int)(blockIdx.x & 1) : 0;
+  const int qchunk = EMAX ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+  if (!tile_of_block(blockIdx.y, flip, TR, TC, lower)) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = (blockIdx.x >> 1) * 32 + lane;
+  const int q = qchunk * 32 + lane;
   const bool q_ok = q < naux;
   __shared__ double rho_sh[8][32];
   __shared__ double dw_sh[32][33];  // weighted density of this tile: (i == j ? 1 : 2) * 0.5 (D_ij + D_ji), 0 above the diagonal
-  if (lower) {
+  if (RHO && lower) {
     for (int idx = threadIdx.x; idx < 1024; idx += 256) {
       const int rl = idx >> 5, cl = idx & 31;
       const int R = TR * 32 + rl, C = TC * 32 + cl;
@@ -122,13 +127,13 @@ __global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict
       }
 #pragma unroll
       for (int cc = 0; cc < 16; ++cc) {
-        hm = max(hm, abs_hi_word(x[cc]));
-        if (lower) rsum = fma(dw_sh[rl][half * 16 + cc], x[cc], rsum);
+        if (EMAX) hm = max(hm, abs_hi_word(x[cc]));
+        if (RHO && lower) rsum = fma(dw_sh[rl][half * 16 + cc], x[cc], rsum);
       }
     }
-    if (q_ok) atomicMax(&emax[(long long)R * naux + q], hm);
+    if (EMAX && q_ok) atomicMax(&emax[(long long)R * naux + q], hm);
   }
-  if (lower) {
+  if (RHO && lower) {
     rho_sh[warp][lane] = rsum;
     __syncthreads();
     if (warp == 0 && q_ok) {
@@ -358,10 +363,19 @@ int64_t jk_rho_part_rows(int nao) { return tile_pairs(nao); }
 
 cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho_part, double* rho,
                              uint32_t* emax, cudaStream_t st) {
-  dim3 grid(2u * (unsigned)((naux + 31) / 32), tile_pairs(nao));
-  jk_pass_a_kernel<<<grid, 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax);
-  jk_rho_reduce_kernel<<<(unsigned)((naux + 31) / 32), 256, 0, st>>>(rho_part, (int)tile_pairs(nao), naux, rho);
-  count_launch(2);
+  const unsigned qchunks = (unsigned)((naux + 31) / 32);
+  if (emax && rho) {
+    jk_pass_a_kernel<true, true><<<dim3(2u * qchunks, tile_pairs(nao)), 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax);
+  } else if (rho) {
+    jk_pass_a_kernel<true, false><<<dim3(qchunks, tile_pairs(nao)), 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax);
+  } else {
+    jk_pass_a_kernel<false, true><<<dim3(2u * qchunks, tile_pairs(nao)), 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax);
+  }
+  count_launch();
+  if (rho) {
+    jk_rho_reduce_kernel<<<qchunks, 256, 0, st>>>(rho_part, (int)tile_pairs(nao), naux, rho);
+    count_launch();
+  }
   return cudaGetLastError();
 }
 

@@ -272,6 +272,76 @@ def test_jk_split_n_tiles(dfe, gpu_ws, s):
     assert dfe.df_last_status() == 0
 
 
+@pytest.mark.parametrize("smax", [4, 8])
+def test_jk_planned_build_bitwise(dfe, gpu_ws, smax):
+    """B split once (row maxima, scale indices, smax digit planes)
+    and reused; a planned build with s <= smax slices reads the first s planes (prefix property,
+    DESIGN.md R3) and must give the bits of df_jk_build -- which the other tests compare with the
+    oracle -- for several (C_occ, D) of an SCF-like sequence, ragged nao, 3 blocks of 512 q."""
+    nao, naux, nocc = 150, 1100, 20
+    Bp = G.make_B_packed(nao, naux, seed=21)
+    Bd = dev(Bp)
+    plan = dfe.Plan(Bd, nao, naux, smax)
+    assert dfe.df_last_status() == 0
+    for it, s in enumerate([2, 3, 4] if smax == 4 else [4, 6, 8]):
+        Cocc = G.make_C_occ(nao, nocc, seed=30 + it)
+        D = G.make_density(Cocc)
+        J = torch.empty((nao, nao), dtype=torch.float64, device=DEV)
+        K = torch.empty_like(J)
+        dfe.df_jk_build_slices(Bd, nao, naux, dev(Cocc), nocc, dev(D), s, J, K)
+        J2 = torch.full_like(J, np.nan)
+        K2 = torch.full_like(K, np.nan)
+        dfe.df_jk_build_planned_slices(plan, Bd, nao, naux, dev(Cocc), nocc, dev(D), s, J2, K2)
+        torch.cuda.synchronize()
+        assert torch.equal(J, J2) and torch.equal(K, K2), s
+        K_emu = O.emul_df_k(Bp, nao, Cocc, s)
+        assert O.rel_frobenius(K2.cpu().numpy(), K_emu) <= 1e-14
+    # tol entry point: same policy as df_jk_build
+    tol = 1e-6
+    dfe.df_jk_build(Bd, nao, naux, dev(Cocc), nocc, dev(D), tol, J, K)
+    if dfe.df_slices_for_tol(tol) <= smax:
+        dfe.df_jk_build_planned(plan, Bd, nao, naux, dev(Cocc), nocc, dev(D), tol, J2, K2)
+        torch.cuda.synchronize()
+        assert torch.equal(J, J2) and torch.equal(K, K2)
+    assert dfe.df_last_status() == 0
+    # more slices than the plan holds, a plan buffer that is too small
+    with pytest.raises(dfe.DFError) as ei:
+        dfe.df_jk_build_planned_slices(plan, Bd, nao, naux, dev(Cocc), nocc, dev(D), smax + 1 if smax < 8 else 9, J2, K2)
+    assert ei.value.code == -3
+    small = torch.empty(dfe.df_jk_plan_bytes(nao, naux, smax) - 1 + 256, dtype=torch.uint8, device=DEV)
+    off = (-small.data_ptr()) % 256
+    rc = dfe.lib.df_jk_plan_create(Bd.data_ptr(), nao, naux, smax, small.data_ptr() + off,
+                                   dfe.df_jk_plan_bytes(nao, naux, smax) - 1, None)
+    assert rc == -4
+    plan.close()
+
+
+def test_jk_planned_small_workspace(dfe, gpu_ws):
+    """A planned build in the planned workspace of one 512-q block (no GEMM(5) planes in it)."""
+    nao, naux, nocc, s = 150, 1100, 20, 5
+    Bp = G.make_B_packed(nao, naux, seed=22)
+    Cocc = G.make_C_occ(nao, nocc, seed=22)
+    D = G.make_density(Cocc)
+    Bd = dev(Bp)
+    J = torch.empty((nao, nao), dtype=torch.float64, device=DEV)
+    K = torch.empty_like(J)
+    dfe.df_jk_build_slices(Bd, nao, naux, dev(Cocc), nocc, dev(D), s, J, K)
+    plan = dfe.Plan(Bd, nao, naux, 6)
+    small = dfe.Workspace(dfe.df_jk_planned_workspace_bytes(nao, naux, nocc, s, 1))
+    try:
+        assert small.view.numel() < dfe.df_jk_workspace_bytes(nao, naux, nocc, s)
+        J2, K2 = torch.empty_like(J), torch.empty_like(K)
+        dfe.df_jk_build_planned_slices(plan, Bd, nao, naux, dev(Cocc), nocc, dev(D), s, J2, K2)
+        torch.cuda.synchronize()
+        with pytest.raises(dfe.DFError) as ei:  # the unplanned build does not fit there
+            dfe.df_jk_build_slices(Bd, nao, naux, dev(Cocc), nocc, dev(D), s, J2.clone(), K2.clone())
+        assert ei.value.code == -4
+    finally:
+        small.close()
+        dfe.df_set_workspace(gpu_ws.view)
+    assert torch.equal(J, J2) and torch.equal(K, K2)
+
+
 def test_jk_workspace_too_small(dfe, gpu_ws):
     tiny = dfe.Workspace(4096)
     try:
@@ -322,8 +392,8 @@ def test_jk_large_config3_sampled(dfe, gpu_ws):
     chunks), sampled J entries, sampled K entries; plus the invariants that hold at any size."""
     torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
-    if free < 75 << 30:
-        pytest.skip("needs ~70 GB of free device memory")
+    if free < 100 << 30:
+        pytest.skip("needs ~90 GB of free device memory")
     cfg = G.CONFIGS["large"]
     nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc
     tol = 2.0 ** -23
@@ -343,7 +413,15 @@ def test_jk_large_config3_sampled(dfe, gpu_ws):
         dfe.df_jk_build(B, nao, naux, dev(Cocc), nocc, dev(D), tol, J2, K2)
         torch.cuda.synchronize()
         assert torch.equal(J, J2) and torch.equal(K, K2)
-        del J2, K2
+        # and a planned build (B split once, 24.6 GB of planes at s = 4) gives the same bits
+        plan = dfe.Plan(B, nao, naux, s)
+        J2.fill_(np.nan); K2.fill_(np.nan)
+        dfe.df_jk_build_planned(plan, B, nao, naux, dev(Cocc), nocc, dev(D), tol, J2, K2)
+        torch.cuda.synchronize()
+        assert dfe.df_last_status() == 0
+        assert torch.equal(J, J2) and torch.equal(K, K2)
+        plan.close()
+        del J2, K2, plan
     finally:
         big.close()
         dfe.df_set_workspace(gpu_ws.view)

@@ -102,6 +102,39 @@ def test_workspace_sizes(dfe):
         dfe.df_jk_workspace_bytes(1200, 4000, 300, 4)  # nocc > 256 unsupported
 
 
+def test_plan_sizes(dfe):
+    """Plan = row maxima + scale indices (4 bytes each per (q, i)) + smax planes of (q, i) rows
+    padded to whole 128-byte lines; a planned build's workspace holds no GEMM(5) operand planes."""
+    rows = 4000 * 1200
+    assert dfe.df_jk_plan_bytes(1200, 4000, 6) == 2 * rows * 4 + 6 * rows * 1280
+    assert dfe.df_jk_plan_bytes(100, 7, 1) == 2 * 2816 + 700 * 128
+    w = dfe.df_jk_workspace_bytes_blocks(1200, 4000, 150, 4, 8)
+    wp = dfe.df_jk_planned_workspace_bytes(1200, 4000, 150, 4, 8)
+    assert 0 < wp <= w - 4 * rows * 1280
+    for bad in ((0, 10, 4), (10, 0, 4), (20000, 10, 4)):
+        with pytest.raises(dfe.DFError) as ei:
+            dfe.df_jk_plan_bytes(*bad)
+        assert ei.value.code == -2
+    for smax in (0, 9):
+        with pytest.raises(dfe.DFError) as ei:
+            dfe.df_jk_plan_bytes(100, 10, smax)
+        assert ei.value.code == -3
+
+
+def test_plan_argument_errors_without_touching_a_device(dfe):
+    lib = dfe.lib
+    assert lib.df_jk_plan_create(None, 4, 4, 4, 256, 1 << 20, None) == -1
+    assert lib.df_jk_plan_create(256, 4, 4, 4, None, 1 << 20, None) == -1
+    assert lib.df_jk_plan_create(256, 0, 4, 4, 256, 1 << 20, None) == -2
+    assert lib.df_jk_plan_create(256, 4, 4, 9, 256, 1 << 20, None) == -3
+    assert lib.df_jk_plan_create(256, 4, 4, 4, 264, 1 << 20, None) == -7
+    assert lib.df_jk_build_planned(None, 4, 1, 4, 4, 1, 1, 1, 1e-6, 1, 1, None) == -1
+    assert lib.df_jk_build_planned_slices(256, 4, 1, 4, 4, 1, 1, 1, 5, 1, 1, None) == -3   # s > smax
+    assert lib.df_jk_build_planned_slices(256, 0, 1, 4, 4, 1, 1, 1, 1, 1, 1, None) == -3   # smax out of range
+    assert lib.df_jk_build_planned_slices(264, 4, 1, 4, 4, 1, 1, 1, 3, 1, 1, None) == -7   # misaligned plan
+    assert lib.df_jk_build_planned_slices(256, 4, 1, 4, 4, 1, 300, 1, 3, 1, 1, None) == -2
+
+
 def test_argument_errors_without_touching_a_device(dfe):
     lib = dfe.lib
     assert lib.df_emul_gemm(None, None, None, 4, 4, 4, 1e-6, None) == -1
@@ -121,6 +154,8 @@ def test_no_cpu_fallback(dfe):
     # valid-looking arguments, no device: the library must refuse, not compute
     assert dfe.lib.df_emul_gemm_slices(256, 256, 256, 4, 4, 4, 3, None) == -5
     assert dfe.lib.df_set_workspace(256, 1 << 20) == -5
+    assert dfe.lib.df_jk_plan_create(256, 4, 4, 4, 256, 1 << 20, None) == -5
+    assert dfe.lib.df_jk_build_planned_slices(256, 4, 256, 4, 4, 256, 1, 256, 3, 256, 256, None) == -5
 
 
 def test_product_does_not_import_oracle():
