@@ -32,12 +32,15 @@ def allreduce_jk(J, K, group=None):
     return J, K
 
 
-def df_jk_build_sharded(B_shard, nao, naux_shard, C_occ, nocc, D, tol, J, K, group=None, stream=None):
+def df_jk_build_sharded(B_shard, nao, naux_shard, C_occ, nocc, D, tol, J, K, group=None, stream=None, plan=None):
     """This rank's df_jk_build over its shard of q (B_shard = B_packed[:, q0:q1], contiguous),
-    then the all-reduce.  With an empty shard the rank contributes zeros."""
+    then the all-reduce.  With an empty shard the rank contributes zeros.  plan: a binding.Plan of
+    this rank's shard (B split once for the whole SCF), or None."""
     from . import binding
 
-    if naux_shard > 0:
+    if naux_shard > 0 and plan is not None:
+        binding.df_jk_build_planned(plan, B_shard, nao, naux_shard, C_occ, nocc, D, tol, J, K, stream)
+    elif naux_shard > 0:
         binding.df_jk_build(B_shard, nao, naux_shard, C_occ, nocc, D, tol, J, K, stream)
     else:
         J.zero_()
