@@ -214,7 +214,10 @@ int df_profile_read(float* ms_by_class, int* count_by_class);
 /* Back-to-back tcgen05.mma.kind::i8 issue-rate probe (operands resident in
  * shared memory, no loads): runs `iters` MMAs of shape 128 x n_mma x 32 per CTA
  * on every SM.  Returns the launch's device time in milliseconds in *ms (host);
- * INT8 op/s = 2*128*n_mma*32*iters*grid / time.  Synchronises. */
+ * INT8 op/s = 2*128*n_mma*32*iters*grid / time.  Synchronises.  n_mma may carry
+ * a number of issuing warps w (1..4, 2*w*N <= 512) in bits 16+: N | w << 16, each
+ * issuing `iters` MMAs into its own accumulators (measured: more issuers do not
+ * raise the rate; an MMA of M = 128 takes max(~50, N/2 + 3) cycles). */
 int df_debug_mma_peak(int n_mma, int iters, int grid, float* ms, void* stream);
 
 #ifdef __cplusplus

@@ -24,7 +24,7 @@ namespace dfe {
 
 constexpr int kMaxStages = 8;
 constexpr int kGemmThreads = 320;  // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue (two per TMEM lane quarter)
-constexpr int kSmemLimit = 232448 - 21504;  // 227 KB minus the static shared memory (barriers, epilogue staging)
+constexpr int kSmemLimit = 232448 - 11264;  // 227 KB minus the static shared memory (barriers, epilogue staging)
 
 struct GemmKernelParams {
   CUtensorMap mapA;
@@ -57,10 +57,11 @@ struct GemmKernelParams {
   uint32_t* xmax;
   int32_t* P;
   int dbg_chunk;
-  // flattened slice-pair list: x = A plane offset>>4 | (B plane offset>>4) << 16 within a stage,
-  // y = accumulator column | (accumulate-from-the-start flag) << 16; pass ps owns
-  // [pass_start[ps], pass_start[ps+1])
-  uint2 pairs[kMaxSlices * (kMaxSlices + 1) / 2];
+  // flattened slice-pair list: x = A plane offset>>4 within a stage, y = B plane offset>>4,
+  // z = accumulator column, w = accumulate-from-the-start flag (one 16-byte constant load and four
+  // uniform adds per MMA: the packed 8-byte form cost 12 uniform instructions per MMA, which at
+  // N = 80 is the MMA's own duration); pass ps owns [pass_start[ps], pass_start[ps+1])
+  uint4 pairs[kMaxSlices * (kMaxSlices + 1) / 2];
   int pass_start[kMaxSlices + 1];
   int dbg_flags;  // bit 0: no MMAs (operand feed only); bit 1: no TMA loads (MMA issue only)
 };
@@ -146,7 +147,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   __shared__ __align__(8) uint64_t tmem_full_bar;
   __shared__ __align__(8) uint64_t tmem_empty_bar;
   __shared__ uint32_t tmem_slot;
-  __shared__ __align__(16) double epi_stage[8][32][10];  // per epilogue warp: 32 rows x 8 cols, 80 B pitch
+  __shared__ __align__(16) double epi_stage[8][16][10];  // per epilogue warp: 16 rows x 8 cols, 80 B pitch
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -204,7 +205,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             const uint32_t ph = (it / S) & 1u;
             mbar_wait(&empty_bar[stage], ph ^ 1u);
             if (p.dbg_flags & 2) {
-              mbar_arrive(&full_bar[stage]);
+              if (CL != 4 || crank == 0) mbar_arrive(&full_bar[stage]);
               continue;
             }
             uint8_t* st = smem + (size_t)stage * p.stage_stride;
@@ -267,7 +268,14 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
           mbar_wait(&full_bar[stage], ph);
           tc_fence_after();
           if (p.dbg_flags & 1) {
-            if (lane == 0) mbar_arrive(&empty_bar[stage]);
+            if (lane == 0) {
+              if (CL == 4 || CL == 2) {
+                mbar_arrive_cluster(mapa_shared(smem_u32(&empty_bar[stage]), 0u));
+                mbar_arrive_cluster(mapa_shared(smem_u32(&empty_bar[stage]), 1u));
+              } else {
+                mbar_arrive(&empty_bar[stage]);
+              }
+            }
             continue;
           }
           const uint32_t lo_base = desc_lo0 | (smem_base16 + stage * stage16);
@@ -279,11 +287,11 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
               const uint32_t later = (kb | kk) ? 1u : 0u;
 #pragma unroll 4
               for (int i = pr0; i < pr1; ++i) {
-                const uint2 e = p.pairs[i];
-                const uint64_t adesc = ((uint64_t)desc_hi << 32) | (lo + (e.x & 0xFFFFu));
-                const uint64_t bdesc = ((uint64_t)desc_hi << 32) | (lo + (e.x >> 16));
-                if (CL == 4) mma_i8_ss_pair(tmem_base + (e.y & 0xFFFFu), adesc, bdesc, idesc, later | (e.y >> 16));
-                else mma_i8_ss(tmem_base + (e.y & 0xFFFFu), adesc, bdesc, idesc, later | (e.y >> 16));
+                const uint4 e = p.pairs[i];
+                const uint64_t adesc = ((uint64_t)desc_hi << 32) | (lo + e.x);
+                const uint64_t bdesc = ((uint64_t)desc_hi << 32) | (lo + e.y);
+                if (CL == 4) mma_i8_ss_pair(tmem_base + e.z, adesc, bdesc, idesc, later | e.w);
+                else mma_i8_ss(tmem_base + e.z, adesc, bdesc, idesc, later | e.w);
               }
             }
             // frees the smem stage once these MMAs have read it (in both CTAs of a pair: the peer
@@ -392,20 +400,26 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
               for (int h = 0; h < 2; ++h) {
                 const long long colv = col0 + c + 8 * h + cpair;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                  double2 v2 = make_double2(0.0, 0.0);
-                  if (srow[j] && colv + 1 < p.b_rows) v2 = *reinterpret_cast<const double2*>(srow[j] + colv);
-                  else if (srow[j] && colv < p.b_rows) v2.x = srow[j][colv];
-                  *reinterpret_cast<double2*>(&stg[(lane >> 2) + 8 * j][cpair]) = v2;
-                }
-                __syncwarp();
+                for (int r = 0; r < 2; ++r) {  // 16 rows per round (the staging tile holds 16)
 #pragma unroll
-                for (int k2 = 0; k2 < 4; ++k2) {
-                  const double2 v2 = *reinterpret_cast<const double2*>(&stg[lane][2 * k2]);
-                  acc[8 * h + 2 * k2] = v2.x;
-                  acc[8 * h + 2 * k2 + 1] = v2.y;
+                  for (int jj = 0; jj < 2; ++jj) {
+                    const int j = 2 * r + jj;
+                    double2 v2 = make_double2(0.0, 0.0);
+                    if (srow[j] && colv + 1 < p.b_rows) v2 = *reinterpret_cast<const double2*>(srow[j] + colv);
+                    else if (srow[j] && colv < p.b_rows) v2.x = srow[j][colv];
+                    *reinterpret_cast<double2*>(&stg[(lane >> 2) + 8 * jj][cpair]) = v2;
+                  }
+                  __syncwarp();
+                  if ((lane >> 4) == r) {
+#pragma unroll
+                    for (int k2 = 0; k2 < 4; ++k2) {
+                      const double2 v2 = *reinterpret_cast<const double2*>(&stg[lane & 15][2 * k2]);
+                      acc[8 * h + 2 * k2] = v2.x;
+                      acc[8 * h + 2 * k2 + 1] = v2.y;
+                    }
+                  }
+                  __syncwarp();
                 }
-                __syncwarp();
               }
             } else {
 #pragma unroll
@@ -443,16 +457,23 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             for (int h = 0; h < 2; ++h) {
               const long long colv = col0 + c + 8 * h + cpair;
 #pragma unroll
-              for (int k2 = 0; k2 < 4; ++k2)
-                *reinterpret_cast<double2*>(&stg[lane][2 * k2]) = make_double2(acc[8 * h + 2 * k2], acc[8 * h + 2 * k2 + 1]);
-              __syncwarp();
+              for (int r = 0; r < 2; ++r) {  // 16 rows per round
+                if ((lane >> 4) == r) {
 #pragma unroll
-              for (int j = 0; j < 4; ++j) {
-                const double2 v2 = *reinterpret_cast<const double2*>(&stg[(lane >> 2) + 8 * j][cpair]);
-                if (srow[j] && colv + 1 < p.b_rows) *reinterpret_cast<double2*>(srow[j] + colv) = v2;
-                else if (srow[j] && colv < p.b_rows) srow[j][colv] = v2.x;
+                  for (int k2 = 0; k2 < 4; ++k2)
+                    *reinterpret_cast<double2*>(&stg[lane & 15][2 * k2]) =
+                        make_double2(acc[8 * h + 2 * k2], acc[8 * h + 2 * k2 + 1]);
+                }
+                __syncwarp();
+#pragma unroll
+                for (int jj = 0; jj < 2; ++jj) {
+                  const int j = 2 * r + jj;
+                  const double2 v2 = *reinterpret_cast<const double2*>(&stg[(lane >> 2) + 8 * jj][cpair]);
+                  if (srow[j] && colv + 1 < p.b_rows) *reinterpret_cast<double2*>(srow[j] + colv) = v2;
+                  else if (srow[j] && colv < p.b_rows) srow[j][colv] = v2.x;
+                }
+                __syncwarp();
               }
-              __syncwarp();
             }
           } else {
 #pragma unroll
@@ -511,7 +532,7 @@ __global__ void __launch_bounds__(128, 1) mma_peak_kernel(int n_mma, int iters, 
   // previous MMA (shared-memory operand bandwidth shows).
   for (int i = threadIdx.x; i < ntiles * (128 + 256) * swz / 4; i += blockDim.x) ((uint32_t*)smem)[i] = 0;
   if (threadIdx.x == 0) {
-    mbar_init(&done_bar, 1);
+    mbar_init(&done_bar, (n_mma >> 16) ? (n_mma >> 16) : 1);
     fence_barrier_init();
   }
   fence_proxy_async();
@@ -520,26 +541,34 @@ __global__ void __launch_bounds__(128, 1) mma_peak_kernel(int n_mma, int iters, 
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_slot;
-  if (warp == 0) {
+  // n_mma = N | (number of issuing warps << 16) (0 = one).  Issuer w accumulates into its own two
+  // TMEM slots; all issuers commit to done_bar.
+  const int nissue = (n_mma >> 16) ? (n_mma >> 16) : 1;
+  n_mma &= 0xFFFF;
+  if (warp < nissue) {
     const uint32_t idesc = make_idesc_i8(128, n_mma);
     const uint64_t proto = make_smem_desc(0, swz);
     const uint32_t a_t16 = 128u * swz / 16u, b_t16 = 256u * swz / 16u, nk = swz / 32;
     const uint32_t hi = (uint32_t)(proto >> 32), lo0 = (uint32_t)proto;
     const uint32_t a16 = (smem_u32(smem) & 0x3FFFFu) >> 4, b16 = a16 + (uint32_t)ntiles * a_t16;
+    const uint32_t slot = tmem_base + (uint32_t)(warp * (512 / nissue));
+    const uint32_t half = (uint32_t)(256 / nissue);
     if (elect_one()) {
       int ta = 0, tb = 0;
+      uint32_t kk2 = 0;
       for (int i = 0; i < iters; ++i) {
-        const uint32_t kk2 = 2u * ((uint32_t)i % nk);  // K step inside the swizzle row, 16-byte units
         const uint64_t adesc = ((uint64_t)hi << 32) | (lo0 | (a16 + (uint32_t)ta * a_t16 + kk2));
         const uint64_t bdesc = ((uint64_t)hi << 32) | (lo0 | (b16 + (uint32_t)tb * b_t16 + kk2));
-        mma_i8_ss(tmem_base + (uint32_t)((i & 1) * 256), adesc, bdesc, idesc, i > 1);
+        mma_i8_ss(slot + (uint32_t)(i & 1) * half, adesc, bdesc, idesc, i > 1);
+        kk2 += 2u;  // K step inside the swizzle row, 16-byte units
+        if (kk2 == 2u * nk) kk2 = 0;
         if (++ta == ntiles) { ta = 0; if (++tb == ntiles) tb = 0; }
       }
       mma_commit(&done_bar);
     }
     __syncwarp();
-    mbar_wait(&done_bar, 0);
   }
+  if (warp == 0) mbar_wait(&done_bar, 0);
   tc_fence_before();
   __syncthreads();
   if (warp == 0) {
@@ -629,7 +658,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   // cta_group::2 pair: 256-row tiles on an SM pair, each CTA holds half of the B tile's N rows --
   // the MMA then reads 6 KB instead of 8 KB of shared memory per 128 x 128 x 32 step
   const bool pair = g.pair && g.n_tile % 32 == 0 && g.mode != kEpiInt32 && g.a_rows > kTileM &&
-                    (!g.lower_only || g.n_tile == 128) && g_gemm_dbg_flags == 0 && !g_gemm_no_pair;
+                    (!g.lower_only || g.n_tile == 128) && !g_gemm_no_pair;
   const int nb = pair ? g.n_tile / 2 : g.n_tile;  // B rows per CTA and stage
   int bk = g.bk;
   if (bk == 0) bk = g_gemm_force_bk;
@@ -702,8 +731,10 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
           any = true;
           next_t[w] = t + 1;
           const uint32_t ao = ((uint32_t)(t - 1) * a_plane) >> 4, bo = (b_off + (uint32_t)(w - t - 1) * b_plane) >> 4;
-          p.pairs[np].x = ao | (bo << 16);
-          p.pairs[np].y = (uint32_t)((slot0 + w_hi - w) * p.acc_stride) | ((t > t_lo ? 1u : 0u) << 16);
+          p.pairs[np].x = ao;
+          p.pairs[np].y = bo;
+          p.pairs[np].z = (uint32_t)((slot0 + w_hi - w) * p.acc_stride);
+          p.pairs[np].w = t > t_lo ? 1u : 0u;
           ++np;
         }
       }
@@ -755,7 +786,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   const size_t smem = (size_t)p.num_stages * p.stage_stride + 1024;
   // cluster pair: the two N tiles of an M tile share the A operand through TMA multicast
   const int cl = pair ? 4
-                 : (g.cluster_n == 2 && p.tiles_n == 2 && !g.lower_only && g_gemm_dbg_flags == 0 && num_sms >= 2) ? 2 : 1;
+                 : (g.cluster_n == 2 && p.tiles_n == 2 && !g.lower_only && num_sms >= 2) ? 2 : 1;
   if (cl == 2) {
     p.group_m = 1;  // work items 2c, 2c+1 = (tm = c, tn = 0 / 1)
     if (!make_plane_map(&p.mapA2, g.A, g.k, g.a_rows, s, g.a_pitch, g.a_plane_stride, bk, 64)) return cudaErrorInvalidValue;
