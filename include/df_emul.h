@@ -131,7 +131,8 @@ int64_t df_jk_planned_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, i
 /* df_jk_build with GEMM(5)'s left operand read from `plan` (created from the same
  * B_packed, nao, naux with `smax` planes; the library cannot check that).  B_packed
  * is still read for rho and J (plain FP64).  Bit-identical to
- * df_jk_build.  DF_ERR_TOL if the slice count exceeds smax. */
+ * df_jk_build.  DF_ERR_TOL if the slice count exceeds smax.  Status bits that B
+ * causes (Inf/NaN, range) are raised by df_jk_plan_create, not again per build. */
 int df_jk_build_planned(const void* plan, int smax, const double* B_packed, int64_t nao, int64_t naux,
                         const double* C_occ, int64_t nocc, const double* D,
                         double tol, double* J, double* K, void* stream);
