@@ -190,54 +190,57 @@ __global__ void __launch_bounds__(256) jk_j_gemv_kernel(const double* __restrict
 }
 
 // Unpack + split.  Output planes[t][(q, R)][C] want C-contiguous 128-byte lines, the input wants
-// q-contiguous runs.  A warp owns one output row R and 8 consecutive q; lane = (qi, cg): q = q8 + qi,
-// columns cg*32 .. cg*32+31 of a 128-column block.  One load instruction reads 64-byte runs of
-// four packed rows; one store instruction writes pieces of only 8 output lines (a fully divergent
-// store costs 32 tag cycles in the LSU, which made the pass store-issue bound), and the four lanes
-// of a q complete its 128-byte line together.  A block = 2 rows x 32 q.  Blocks are ordered
-// [128 x 128 super-tile pair (A >= B)][q chunk][sub]: sub 0..63 = row pairs of the (A, B) block
-// (rows in A, columns in B), sub 64..127 = the mirrored (B, A) block; both read the same 128 x 128
-// packed rows of this q chunk (4 MB) back to back, so the second read is an L2 hit.
+// q-contiguous runs; the block transposes through shared memory so that both are whole lines.
+// A block owns kUnpackRows consecutive output rows R of one 128 x 128 tile, 32 consecutive q and
+// the tile's 128 columns: lane = q, warp = 16-column group.  Per row a thread loads its 16 values
+// (a warp instruction reads one 256-byte run of a packed row), converts them with the scale of
+// (q, R), and writes 16 bytes per plane into the staging tile [plane][q][128 + 16 pad]; after one
+// barrier (the tile is double buffered) the warps copy it out, 8 lanes per 128-byte line of
+// (plane, q, R).  Blocks are ordered [128 x 128 super-tile pair (A >= B)][q chunk][sub]: the first
+// half of the subs are the row groups of the (A, B) block (rows in A, columns in B), the second
+// half those of the mirrored (B, A) block; both read the same 128 x 128 packed rows of this q
+// chunk (4 MB) back to back, so the second read is an L2 hit.  Two rows per block keep the number
+// of tiles in flight, and with it the L2 working set, small (8 rows: 11.2 / 16.9 ms at s = 4 / 6
+// against 10.5 / 14.3 ms).  Four resident blocks per SM up to s = 4, three above (measured both ways).
+constexpr int kUnpackRows = 2;
+constexpr int kUnpackPitch = 144;  // staging row: 128 bytes + 16 (conflict-free 16-byte stores by 8 lanes)
 template <int S>
-__global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __restrict__ Bp, int nao, int naux,
+__global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(const double* __restrict__ Bp, int nao, int naux,
                                                               int q0, int q1, const uint32_t* __restrict__ emax,
                                                               int32_t* __restrict__ e5, int8_t* __restrict__ planes,
                                                               long long pitch, long long plane_stride,
                                                               int* __restrict__ status, int dbg) {
+  extern __shared__ __align__(16) uint8_t ubuf[];  // [2][S][32][kUnpackPitch]
+  constexpr int kSubs = 128 / kUnpackRows;
   int A, B;
   bool lower;
-  const int sub = blockIdx.x & 127;
-  if (!tile_of_block(blockIdx.y, sub >> 6, A, B, lower)) return;  // (A, B) = (row block, column block)
+  const int sub = (int)(blockIdx.x % (2 * kSubs));
+  const int chunk = (int)(blockIdx.x / (2 * kSubs));
+  if (!tile_of_block(blockIdx.y, sub / kSubs, A, B, lower)) return;  // (A, B) = (row block, column block)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int R = A * 128 + (sub & 63) * 2 + (warp >> 2);
-  const int q = q0 + (blockIdx.x >> 7) * 32 + (warp & 3) * 8 + (lane >> 2);
-  // a thread owns columns [C0, C0 + 16) and [C0 + 64, C0 + 80): the four lanes of a q write 64
-  // contiguous bytes per store instruction (whole sectors); pitch is a multiple of 128
-  const int C0 = B * 128 + (lane & 3) * 16;
-  if (R >= nao || q >= q1) return;
-  const uint32_t hm = emax[(long long)R * naux + q];
-  const int e = scale_index_from_hi(hm);
-  const long long orow = (long long)(q - q0) * nao + R;
-  if (lower && C0 == 0) {
-    e5[orow] = e;
-    const int stt = status_from_hi(hm);
-    if (stt) atomicOr(status, stt);
-  }
-  const double scale = pow2_double(63 - e);
+  const int qg = q0 + chunk * 32 + lane;
+  const bool q_ok = qg < q1;
+  const int q = q_ok ? qg : q1 - 1;  // a valid address; the lane's results are dropped
+  const int Cs = B * 128 + warp * 16;
   const char* bq = reinterpret_cast<const char*>(Bp + q);
   const unsigned naux8 = (unsigned)naux * 8u;
   // block-uniform shape of the tile: rows in block A, columns in block B
   const int kind = (A > B) ? 0 : (A < B) ? 1 : 2;
   const bool full = B * 128 + 128 <= nao;
-  int8_t* const orow_ptr = planes + orow * pitch + C0;
-  // all 16 loads of a half are issued before the first conversion; everything is stored at the end
-  // (storing each half before loading the next one, at 4 blocks per SM, ran 35 % slower: 15.6 ms
-  // against 11.5 ms although loads alone and stores alone were both faster)
-  uint32_t w[S][8];
-#pragma unroll
-  for (int half = 0; half < 2; ++half) {
+  const int nq_blk = min(32, q1 - (q0 + chunk * 32));
+#pragma unroll 1
+  for (int r = 0; r < kUnpackRows; ++r) {
+    const int R = A * 128 + (sub % kSubs) * kUnpackRows + r;
+    if (R >= nao) break;  // block-uniform
+    const uint32_t hm = emax[(long long)R * naux + q];
+    const int e = scale_index_from_hi(hm);
+    if (lower && B == 0 && warp == 0 && q_ok) {
+      e5[(long long)(qg - q0) * nao + R] = e;
+      const int stt = status_from_hi(hm);
+      if (stt) atomicOr(status, stt);
+    }
+    const double scale = pow2_double(63 - e);
     double x[16];
-    const int Cs = C0 + half * 64;
     if (dbg & 2) {
 #pragma unroll
       for (int cc = 0; cc < 16; ++cc) x[cc] = 0.0;
@@ -249,6 +252,7 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
       if (kind == 1) load_row16<1, false>(x, bq, naux8, R, Cs, nao);
       else load_row16<2, false>(x, bq, naux8, R, Cs, nao);  // kind 0 has B < A: always full
     }
+    uint32_t w[S][4];
 #pragma unroll
     for (int g4 = 0; g4 < 4; ++g4) {
       uint32_t hi[4], lo[4], ph[4], pl[4];
@@ -261,15 +265,22 @@ __global__ void __launch_bounds__(256) jk_unpack_split_kernel(const double* __re
       transpose4x4_bytes(hi, ph);
       if (S > 4) transpose4x4_bytes(lo, pl);
 #pragma unroll
-      for (int t = 0; t < S; ++t) w[t][half * 4 + g4] = (t < 4) ? ph[3 - t] : pl[7 - t];
+      for (int t = 0; t < S; ++t) w[t][g4] = (t < 4) ? ph[3 - t] : pl[7 - t];
     }
-  }
+    uint8_t* const buf = ubuf + (size_t)(r & 1) * (S * 32 * kUnpackPitch);
 #pragma unroll
-  for (int t = 0; t < S; ++t) {
-    if ((dbg & 1) && w[t][0] != 0x12345678u) continue;
-    uint4* dst = reinterpret_cast<uint4*>(orow_ptr + t * plane_stride);
-    dst[0] = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
-    dst[4] = make_uint4(w[t][4], w[t][5], w[t][6], w[t][7]);
+    for (int t = 0; t < S; ++t)
+      *reinterpret_cast<uint4*>(buf + (t * 32 + lane) * kUnpackPitch + warp * 16) =
+          make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+    __syncthreads();  // one barrier per row: buffer (r + 1) & 1 was last read before this barrier
+    if (dbg & 1) continue;
+    const long long row0 = ((long long)chunk * 32 * nao + R) * pitch + B * 128 + (lane & 7) * 16;
+    for (int idx = warp * 4 + (lane >> 3); idx < S * 32; idx += 32) {
+      const int t = idx >> 5, qq = idx & 31;
+      if (qq < nq_blk)
+        *reinterpret_cast<uint4*>(planes + t * plane_stride + row0 + (long long)qq * nao * pitch) =
+            *reinterpret_cast<const uint4*>(buf + (t * 32 + qq) * kUnpackPitch + (lane & 7) * 16);
+    }
   }
 }
 
@@ -398,14 +409,33 @@ cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const do
     default: { constexpr int SS = 8; CALL; } break; \
   }
 
+template <int S>
+static cudaError_t unpack_split_s(dim3 grid, int smem, cudaStream_t st, const double* Bp, int nao, int naux, int q0,
+                                  int q1, const uint32_t* emax, int32_t* e5, int8_t* planes5, int64_t pitch,
+                                  int64_t plane_stride, int* status) {
+  static bool attr_set = false;  // one opt-in per instantiation (s >= 6 stages more than 48 KB)
+  if (!attr_set) {
+    cudaError_t err = cudaFuncSetAttribute(jk_unpack_split_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           2 * S * 32 * kUnpackPitch);
+    if (err != cudaSuccess) return err;
+    attr_set = true;
+  }
+  jk_unpack_split_kernel<S><<<grid, 256, smem, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5, pitch, plane_stride,
+                                                     status, g_jk_dbg);
+  return cudaSuccess;
+}
+
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
                                    int* status, cudaStream_t st) {
   const unsigned T128 = (unsigned)((nao + 127) / 128);
   if (pitch % 128 != 0 || pitch < 128 * (int64_t)T128) return cudaErrorInvalidValue;
-  dim3 grid(128u * (unsigned)((q1 - q0 + 31) / 32), T128 * (T128 + 1) / 2);
-  DFE_DISPATCH_S(s, (jk_unpack_split_kernel<SS><<<grid, 256, 0, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5,
-                                                                      pitch, plane_stride, status, g_jk_dbg)));
+  dim3 grid((unsigned)(2 * (128 / kUnpackRows)) * (unsigned)((q1 - q0 + 31) / 32), T128 * (T128 + 1) / 2);
+  const int smem = 2 * s * 32 * kUnpackPitch;
+  cudaError_t err = cudaSuccess;
+  DFE_DISPATCH_S(s, (err = unpack_split_s<SS>(grid, smem, st, Bp, nao, naux, q0, q1, emax, e5, planes5, pitch,
+                                              plane_stride, status)));
+  if (err != cudaSuccess) return err;
   count_launch();
   return cudaGetLastError();
 }
