@@ -701,9 +701,11 @@ int df_profile_read(float* ms_by_class, int* count_by_class) {
 
 int df_debug_mma_peak(int n_mma, int iters, int grid, float* ms, void* stream) {
   if (!ms) return DF_ERR_NULL;
-  const int n = n_mma & 0xFFFF, nissue = n_mma >> 16;  // N | issuing warps << 16 (0 = one)
+  // N | issuing warps << 16 (0 = one) | pair probe << 24 (cta_group::2, M = 256, one issuer)
+  const int n = n_mma & 0xFFFF, nissue = (n_mma >> 16) & 0xFF, pairp = (n_mma >> 24) & 1;
   if (n < 16 || n > 256 || (n % 16) != 0 || iters < 2 || grid < 1) return DF_ERR_DIM;
   if (nissue < 0 || nissue > 4 || 2 * (nissue ? nissue : 1) * n > 512) return DF_ERR_DIM;
+  if (pairp && (nissue != 0 || grid < 2 || (n % 32) != 0)) return DF_ERR_DIM;
   if (!device_ok()) return DF_ERR_DEVICE;
   if (launch_mma_peak(n_mma, iters, grid, ms, (cudaStream_t)stream) != cudaSuccess) return DF_ERR_CUDA;
   return DF_OK;
