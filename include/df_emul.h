@@ -218,7 +218,8 @@ int df_profile_read(float* ms_by_class, int* count_by_class);
  * INT8 op/s = 2*128*n_mma*32*iters*grid / time.  Synchronises.  n_mma may carry
  * a number of issuing warps w (1..4, 2*w*N <= 512) in bits 16+: N | w << 16, each
  * issuing `iters` MMAs into its own accumulators (measured: more issuers do not
- * raise the rate; an MMA of M = 128 takes max(~50, N/2 + 3) cycles). */
+ * raise the rate; an MMA of M = 128 takes max(~50, N/2 + 3) cycles).  Bit 24 set
+ * (N % 32 == 0, grid >= 2): the same on SM pairs, cta_group::2 MMAs of M = 256. */
 int df_debug_mma_peak(int n_mma, int iters, int grid, float* ms, void* stream);
 
 #ifdef __cplusplus

@@ -272,6 +272,25 @@ def test_jk_split_n_tiles(dfe, gpu_ws, s):
     assert dfe.df_last_status() == 0
 
 
+@pytest.mark.parametrize("s", [1, 2, 3, 4, 5, 6, 7, 8])
+def test_jk_every_slice_count_ragged(dfe, gpu_ws, s):
+    """Every template instantiation of the unpack / split kernels (s = 1..8) on a ragged case:
+    nao = 137 (one full 128-tile + 9 rows, last 16-column group partial), naux = 77 (two full
+    32-q chunks + 13), nocc = 21 (a_pad 32).  GEMM(5) output bit-exact, K up to summation order."""
+    nao, naux, nocc = 137, 77, 21
+    Bp = G.make_B_packed(nao, naux, seed=40 + s)
+    Cocc = G.make_C_occ(nao, nocc, seed=40 + s)
+    D = G.make_density(Cocc)
+    J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+    K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
+    J_ref, _ = O.df_jk_plain(Bp, nao, Cocc, D)
+    assert np.array_equal(X[:, :, :nocc], X_emu)
+    assert not X[:, :, nocc:].any()
+    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert O.rel_frobenius(J, J_ref) <= 1e-12
+    assert np.array_equal(K, K.T) and dfe.df_last_status() == 0
+
+
 @pytest.mark.parametrize("smax", [4, 8])
 def test_jk_planned_build_bitwise(dfe, gpu_ws, smax):
     """B split once (row maxima, scale indices, smax digit planes)
