@@ -429,13 +429,34 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
               }
             }
           }
-          for (int w = w_hi; w >= w_lo; --w) {
-            tmem_ld16(t_lane + (uint32_t)((slot0 + w_hi - w) * p.acc_stride + c), v);
-            tmem_ld_wait();
-            const int eb = eA + 2 - 8 * w;
+          if (first) {
+            // Nothing accumulated yet: sum_w 2^(eb_w) P_w, w descending, in Horner form
+            // t = P_whi; t = fma(t, 2^-8, P_w); acc = t 2^(eb_wlo).  The scale factors are exact
+            // powers of two, so every rounding is the rounding of the running sum of R6 scaled by one:
+            // the same bits with one multiply-add per term and one scale per element.
+            for (int w = w_hi; w >= w_lo; --w) {
+              tmem_ld16(t_lane + (uint32_t)((slot0 + w_hi - w) * p.acc_stride + c), v);
+              tmem_ld_wait();
+              if (w == w_hi) {
 #pragma unroll
-            for (int j = 0; j < 16; ++j)
-              acc[j] = fma((double)(int32_t)v[j], pow2_double(eb + eBv[j]), acc[j]);
+                for (int j = 0; j < 16; ++j) acc[j] = (double)(int32_t)v[j];
+              } else {
+#pragma unroll
+                for (int j = 0; j < 16; ++j) acc[j] = fma(acc[j], 0x1p-8, (double)(int32_t)v[j]);
+              }
+            }
+            const int eb = eA + 2 - 8 * w_lo;
+#pragma unroll
+            for (int j = 0; j < 16; ++j) acc[j] *= pow2_double(eb + eBv[j]);
+          } else {
+            for (int w = w_hi; w >= w_lo; --w) {
+              tmem_ld16(t_lane + (uint32_t)((slot0 + w_hi - w) * p.acc_stride + c), v);
+              tmem_ld_wait();
+              const int eb = eA + 2 - 8 * w;
+#pragma unroll
+              for (int j = 0; j < 16; ++j)
+                acc[j] = fma((double)(int32_t)v[j], pow2_double(eb + eBv[j]), acc[j]);
+            }
           }
           if (last && row_ok) {
 #pragma unroll
