@@ -199,8 +199,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
           int w_hi, w_lo, slot0;
           pass_weights(p, ps, w_hi, w_lo, slot0);
           const int P = min(s, w_hi - 1);
-          const uint32_t tx = (uint32_t)P * (a_plane_bytes + b_plane_bytes);
-          for (int kb = 0; kb < nkb; ++kb, ++it) {
+          // a pass that needs P < s planes packs kp = s / P consecutive K blocks into one stage
+          // (K block j of plane t in plane slot j P + t): fewer, fuller stages -- the one-plane
+          // pass of a two-pass tile was waiting 1230 cycles per K block for 4 MMAs
+          const int kp = s / P;
+          const int nst = (nkb + kp - 1) / kp;
+          for (int sb = 0; sb < nst; ++sb, ++it) {
             const uint32_t stage = it % S;
             const uint32_t ph = (it / S) & 1u;
             mbar_wait(&empty_bar[stage], ph ^ 1u);
@@ -209,29 +213,37 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
               continue;
             }
             uint8_t* st = smem + (size_t)stage * p.stage_stride;
-            const int kpos = kc0 + kb * BK;
+            const int nj = min(kp, nkb - sb * kp);  // K blocks in this stage
+            const uint32_t tx = (uint32_t)(nj * P) * (a_plane_bytes + b_plane_bytes);
             if (CL == 4) {
               // both CTAs' loads count on the LEADER's full barrier, which expects the bytes of both
               const uint32_t lead_bar = mapa_shared(smem_u32(&full_bar[stage]), 0u);
               if (crank == 0) mbar_expect_tx(&full_bar[stage], 2u * tx);
-              for (int t = 0; t < P; ++t)
-                tma_load_3d_pair(st + t * a_plane_bytes, &p.mapA, lead_bar, kpos, tm * kTileM, t);
-              for (int u = 0; u < P; ++u)
-                tma_load_3d_pair(st + b_off + u * b_plane_bytes, &p.mapBh, lead_bar, kpos,
-                                 tn * p.n_tile + (int)crank * (p.n_tile / 2), u);
+              for (int j = 0; j < nj; ++j) {
+                const int kpos = kc0 + (sb * kp + j) * BK;
+                for (int t = 0; t < P; ++t)
+                  tma_load_3d_pair(st + (j * P + t) * a_plane_bytes, &p.mapA, lead_bar, kpos, tm * kTileM, t);
+                for (int u = 0; u < P; ++u)
+                  tma_load_3d_pair(st + b_off + (j * P + u) * b_plane_bytes, &p.mapBh, lead_bar, kpos,
+                                   tn * p.n_tile + (int)crank * (p.n_tile / 2), u);
+              }
               continue;
             }
             mbar_expect_tx(&full_bar[stage], tx);
-            if (CL == 2) {
-              for (int t = 0; t < P; ++t)
-                tma_load_3d_mcast(st + t * a_plane_bytes + crank * (64 * BK), &p.mapA2, &full_bar[stage], kpos,
-                                  tm * kTileM + (int)crank * 64, t, (uint16_t)3);
-            } else {
-              for (int t = 0; t < P; ++t)
-                tma_load_3d(st + t * a_plane_bytes, &p.mapA, &full_bar[stage], kpos, tm * kTileM, t);
+            for (int j = 0; j < nj; ++j) {
+              const int kpos = kc0 + (sb * kp + j) * BK;
+              if (CL == 2) {
+                for (int t = 0; t < P; ++t)
+                  tma_load_3d_mcast(st + (j * P + t) * a_plane_bytes + crank * (64 * BK), &p.mapA2, &full_bar[stage],
+                                    kpos, tm * kTileM + (int)crank * 64, t, (uint16_t)3);
+              } else {
+                for (int t = 0; t < P; ++t)
+                  tma_load_3d(st + (j * P + t) * a_plane_bytes, &p.mapA, &full_bar[stage], kpos, tm * kTileM, t);
+              }
+              for (int u = 0; u < P; ++u)
+                tma_load_3d(st + b_off + (j * P + u) * b_plane_bytes, &p.mapB, &full_bar[stage], kpos,
+                            tn * p.n_tile, u);
             }
-            for (int u = 0; u < P; ++u)
-              tma_load_3d(st + b_off + u * b_plane_bytes, &p.mapB, &full_bar[stage], kpos, tn * p.n_tile, u);
           }
         }
       }
@@ -262,7 +274,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
           mbar_wait(&tmem_empty_bar, (iter - 1) & 1u);
           tc_fence_after();
         }
-        for (int kb = 0; kb < nkb; ++kb, ++it) {
+        int w_hi_p, w_lo_p, slot0_p;
+        pass_weights(p, ps, w_hi_p, w_lo_p, slot0_p);
+        const int P = min(s, w_hi_p - 1);
+        const int kp = s / P;  // K blocks per stage (see the producer)
+        const int nst = (nkb + kp - 1) / kp;
+        const uint32_t a_sub16 = (uint32_t)P * (a_plane_bytes >> 4), b_sub16 = (uint32_t)P * (b_plane_bytes >> 4);
+        for (int sb = 0; sb < nst; ++sb, ++it) {
           const uint32_t stage = it % S;
           const uint32_t ph = (it / S) & 1u;
           mbar_wait(&full_bar[stage], ph);
@@ -279,19 +297,24 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             continue;
           }
           const uint32_t lo_base = desc_lo0 | (smem_base16 + stage * stage16);
-          const int kpos = kc0 + kb * BK;
-          const int nkk = (min(BK, kc1 - kpos) + 31) / 32;
+          const int nj = min(kp, nkb - sb * kp);
           if (elect_one()) {
-            for (int kk = 0; kk < nkk; ++kk) {
-              const uint32_t lo = lo_base + 2u * kk;  // +32 bytes per K step, in 16-byte units
-              const uint32_t later = (kb | kk) ? 1u : 0u;
+            for (int j = 0; j < nj; ++j) {
+              const int kb = sb * kp + j;
+              const int kpos = kc0 + kb * BK;
+              const int nkk = (min(BK, kc1 - kpos) + 31) / 32;
+              const uint32_t aj = (uint32_t)j * a_sub16, bj = (uint32_t)j * b_sub16;
+              for (int kk = 0; kk < nkk; ++kk) {
+                const uint32_t lo = lo_base + 2u * kk;  // +32 bytes per K step, in 16-byte units
+                const uint32_t later = (kb | kk) ? 1u : 0u;
 #pragma unroll 4
-              for (int i = pr0; i < pr1; ++i) {
-                const uint4 e = p.pairs[i];
-                const uint64_t adesc = ((uint64_t)desc_hi << 32) | (lo + e.x);
-                const uint64_t bdesc = ((uint64_t)desc_hi << 32) | (lo + e.y);
-                if (CL == 4) mma_i8_ss_pair(tmem_base + e.z, adesc, bdesc, idesc, later | e.w);
-                else mma_i8_ss(tmem_base + e.z, adesc, bdesc, idesc, later | e.w);
+                for (int i = pr0; i < pr1; ++i) {
+                  const uint4 e = p.pairs[i];
+                  const uint64_t adesc = ((uint64_t)desc_hi << 32) | (lo + e.x + aj);
+                  const uint64_t bdesc = ((uint64_t)desc_hi << 32) | (lo + e.y + bj);
+                  if (CL == 4) mma_i8_ss_pair(tmem_base + e.z, adesc, bdesc, idesc, later | e.w);
+                  else mma_i8_ss(tmem_base + e.z, adesc, bdesc, idesc, later | e.w);
+                }
               }
             }
             // frees the smem stage once these MMAs have read it (in both CTAs of a pair: the peer
