@@ -24,7 +24,7 @@ namespace dfe {
 
 constexpr int kMaxStages = 8;
 constexpr int kGemmThreads = 320;  // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue (two per TMEM lane quarter)
-constexpr int kSmemLimit = 232448 - 11264;  // 227 KB minus the static shared memory (barriers, epilogue staging)
+constexpr int kSmemLimit = 232448 - 13312;  // 227 KB minus the static shared memory (barriers, epilogue staging)
 
 struct GemmKernelParams {
   CUtensorMap mapA;
@@ -148,6 +148,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   __shared__ __align__(8) uint64_t tmem_empty_bar;
   __shared__ uint32_t tmem_slot;
   __shared__ __align__(16) double epi_stage[8][16][10];  // per epilogue warp: 16 rows x 8 cols, 80 B pitch
+  __shared__ int eb_sh[2][256];  // scale indices of the tile's columns (double buffered over tiles)
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -337,8 +338,18 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   } else {
     // ================= epilogue: TMEM -> FP64 recombination -> global =================
     const int quarter = warp & 3;
-    uint32_t iter = 0;
+    uint32_t iter = 0, tile_no = 0;
     DFE_WORK_LOOP
+    // the column scale indices of this tile, staged once by the 256 epilogue threads (they were 16
+    // global loads at the head of every 16-column chunk, on the epilogue's critical path)
+    int* const ebs = eb_sh[tile_no & 1u];
+    ++tile_no;
+    {
+      const int et = (warp - 2) * 32 + lane;
+      const long long col = (long long)tn * p.n_tile + et;
+      ebs[et] = (p.mode != kEpiInt32 && et < p.n_tile && col < p.b_rows) ? p.eB[z * p.eb_stride + col] : 0;
+      asm volatile("bar.sync 1, 256;" ::: "memory");  // epilogue warps only; buffer tile_no & 1 is free again
+    }                                                  // once every warp has passed the next tile's barrier
     const int row_local = quarter * 32 + lane;
     const long long row = (long long)tm * kTileM + row_local;
     const bool row_ok = row < p.a_rows;
@@ -403,8 +414,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
           int eBv[16];
 #pragma unroll
           for (int j = 0; j < 16; ++j) {
-            const long long col = col0 + c + j;
-            eBv[j] = (row_ok && col < p.b_rows) ? p.eB[z * p.eb_stride + col] : 0;
+            eBv[j] = row_ok ? ebs[c + j] : 0;
             acc[j] = 0.0;
           }
           if (!first && p.tp) {
