@@ -541,9 +541,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         tc_fence_before();
         if (CL == 4) {  // one arrival per warp on the leader's barrier
           __syncwarp();
-          if (lane == 0) mbar_arrive_cluster(mapa_shared(smem_u32(&tmem_empty_bar), 0u));
+          if (lane == 0) mbar_arrive_cluster_relaxed(mapa_shared(smem_u32(&tmem_empty_bar), 0u));
         } else {
-          mbar_arrive(&tmem_empty_bar);
+          mbar_arrive_relaxed(&tmem_empty_bar);
         }
       }
     }
