@@ -195,7 +195,8 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
  *   bit 4 / 5  unpack kernel writes nothing / reads nothing   bit 6  GEMM(5) N halves without the
  *                                                                    cluster-pair multicast
  *   bits 8-15  force the K-block width in bytes (32, 64, 128) bits 16-19 MMA probe: operand tiles
- *   bit 20     no cta_group::2 pair tiles                            walked (2 bits), swizzle (2 bits) */
+ *   bit 20     no cta_group::2 pair tiles                            walked (2 bits), swizzle (2 bits)
+ *   bit 22     GEMM(5) N halves on multicast CTA pairs, never on MMA pairs */
 int df_debug_set_gemm_flags(int flags);
 
 /* Number of GPU kernels this library has launched in this process. */

@@ -22,6 +22,7 @@ static int g_mode = DF_MODE_GUARDED;
 static int g_device_ok = -1;
 static int g_g5_split_n = 1;
 static int g_g5_cluster = 1;
+static int g_g5_pair_halves = 1;
 
 // ---- optional per-kernel-class CUDA-event timing (df_profile_*; bench.py's roofline) ----
 enum ProfClass { kPSplit = 0, kPPassA, kPJGemv, kPUnpack, kPGemm5, kPSplitX, kPGemm6, kPReduce, kPGemm, kPNum };
@@ -369,11 +370,16 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
         g5.pair = 1;
       } else if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) {
         g5.n_tile = w.a_pad / 2;
+        // one pass per half (all s accumulators in TMEM): the halves run as 256-row tiles on MMA pairs
+        // (an MMA costs at least ~50 cycles per 128 rows whatever N, and a pair instruction covers
+        // 256) -- 13.6 / 17.6 ms against 14.6 / 21.9 ms at s = 5 / 6 for the multicast pair below;
+        // with several passes (s >= 7 at nocc = 150) the two are equal
+        if (g_g5_pair_halves && (int64_t)s * g5.n_tile <= 512) g5.pair = 1;
       }
     }
     g5.acc_stride = (g5.n_tile % 32) ? g5.n_tile : 0;
     g5.x_cols = w.a_pad;
-    g5.cluster_n = (g_g5_cluster && g5.n_tile * 2 == w.a_pad) ? 2 : 1;
+    g5.cluster_n = (g_g5_cluster && g5.n_tile * 2 == w.a_pad && !g5.pair) ? 2 : 1;
     g5.nz = 1;
     g5.eA = planned ? reinterpret_cast<const int32_t*>(plan_b + PL.e5_off) + qs0 * nao : w.e5;
     g5.eB = w.eC;
@@ -664,6 +670,7 @@ int df_debug_set_gemm_flags(int flags) {
   g_g5_split_n = (flags & 4) ? 0 : 1;  // bit 2: GEMM(5) keeps one N tile
   g_g5_cluster = (flags & 64) ? 0 : 1;  // bit 6: GEMM(5) N halves without the multicast pair
   set_jk_debug_flags((flags >> 4) & 3);  // bits 4, 5: unpack kernel without stores / without loads
+  g_g5_pair_halves = ((flags >> 22) & 1) ? 0 : 1;  // bit 22: GEMM(5) N halves never on MMA pairs
   set_peak_tiles((flags >> 16) & 15);  // bits 16-19: MMA probe operand tiles / swizzle
   return DF_OK;
 }

@@ -804,7 +804,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   const int s = g.s;
   // cta_group::2 pair: 256-row tiles on an SM pair, each CTA holds half of the B tile's N rows --
   // the MMA then reads 6 KB instead of 8 KB of shared memory per 128 x 128 x 32 step
-  const bool pair = g.pair && g.n_tile % 32 == 0 && g.mode != kEpiInt32 && g.a_rows > kTileM &&
+  const bool pair = g.pair && g.n_tile % 16 == 0 && g.mode != kEpiInt32 && g.a_rows > kTileM &&
                     (!g.lower_only || g.n_tile == 128) && !g_gemm_no_pair;
   const int nb = pair ? g.n_tile / 2 : g.n_tile;  // B rows per CTA and stage
   int bk = g.bk;
