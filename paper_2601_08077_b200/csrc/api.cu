@@ -366,7 +366,8 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
       const int W0 = 512 / (int)round_up(w.a_pad, 32);
       if (s == W0 + 1 && W0 >= 3 && w.a_pad % 32 == 0 && g_g5_split_n) {
         // one more weight than TMEM slots: the whole a_pad on cta_group::2 pairs, second pass (one
-        // weight) with the running sum parked in TMEM -- 11.9 vs 12.9 ms at nocc = 150, s = 4
+        // weight) with the running sum parked in TMEM -- 9.3-10.5 ms at nocc = 150, s = 4, against
+        // 10.8-11.5 ms for two single-pass halves on MMA pairs (A streamed twice)
         g5.pair = 1;
       } else if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) {
         g5.n_tile = w.a_pad / 2;
