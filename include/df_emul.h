@@ -196,7 +196,8 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
  *                                                                    cluster-pair multicast
  *   bits 8-15  force the K-block width in bytes (32, 64, 128) bits 16-19 MMA probe: operand tiles
  *   bit 20     no cta_group::2 pair tiles                            walked (2 bits), swizzle (2 bits)
- *   bit 22     GEMM(5) N halves on multicast CTA pairs, never on MMA pairs */
+ *   bit 22     GEMM(5) N halves on multicast CTA pairs, never on MMA pairs
+ *   bit 23     GEMM epilogue moves FP64 through the staged 16-byte path, never 256-bit accesses */
 int df_debug_set_gemm_flags(int flags);
 
 /* Number of GPU kernels this library has launched in this process. */

@@ -63,7 +63,7 @@ struct GemmKernelParams {
   // N = 80 is the MMA's own duration); pass ps owns [pass_start[ps], pass_start[ps+1])
   uint4 pairs[kMaxSlices * (kMaxSlices + 1) / 2];
   int pass_start[kMaxSlices + 1];
-  int dbg_flags;  // bit 0: no MMAs (operand feed only); bit 1: no TMA loads (MMA issue only)
+  int dbg_flags;  // bit 0: no MMAs (operand feed only); bit 1: no TMA loads (MMA issue only); bit 2: no 256-bit epilogue accesses
 };
 
 // weights of pass `ps`: w_hi down to w_lo; weight w accumulates in TMEM slot slot0 + (w_hi - w)
@@ -373,6 +373,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     const long long ld_out = (p.mode == kEpiX) ? p.ldx : p.ldc;
     const bool vec_ok = p.mode != kEpiInt32 && ((ld_out | p.c_stride | (long long)col0) & 1) == 0 &&
                         ((uintptr_t)p.C & 15) == 0;
+    // whole 32-byte sectors per lane (256-bit accesses): the thread's own row, no transposition
+    const bool v4_ok = vec_ok && ((ld_out | p.c_stride | (long long)col0) & 3) == 0 && ((uintptr_t)p.C & 31) == 0 &&
+                       !(p.dbg_flags & 4);
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       const long long rr = (long long)tm * kTileM + quarter * 32 + (lane >> 2) + 8 * j;
@@ -426,9 +429,24 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
 #pragma unroll
             for (int j = 0; j < 16; ++j) acc[j] = __hiloint2double((int)v[j], (int)plo[j]);
           } else if (!first) {
-            // running sum of the earlier passes/chunks: coalesced 16-byte loads (4 lanes cover 64
-            // bytes of a row), transposed through shared memory to "lane = row"
-            if (vec_ok) {
+            // running sum of the earlier passes/chunks: one 32-byte sector per lane and load, or
+            // coalesced 16-byte loads (4 lanes cover 64 bytes of a row), transposed through shared
+            // memory to "lane = row"
+            if (v4_ok) {
+              if (row_ok) {
+#pragma unroll
+                for (int k4 = 0; k4 < 4; ++k4) {
+                  const long long colv = col0 + c + 4 * k4;
+                  if (colv + 3 < p.b_rows) {
+                    ld_global_v4f64(out + colv, acc[4 * k4], acc[4 * k4 + 1], acc[4 * k4 + 2], acc[4 * k4 + 3]);
+                  } else {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                      if (colv + j < p.b_rows) acc[4 * k4 + j] = out[colv + j];
+                  }
+                }
+              }
+            } else if (vec_ok) {
 #pragma unroll
               for (int h = 0; h < 2; ++h) {
                 const long long colv = col0 + c + 8 * h + cpair;
@@ -506,6 +524,20 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             }
             tmem_st16(t_lane + (uint32_t)c, plo);
             tmem_st16(t_lane + (uint32_t)(p.acc_stride + c), v);
+          } else if (v4_ok) {
+            if (row_ok) {
+#pragma unroll
+              for (int k4 = 0; k4 < 4; ++k4) {
+                const long long colv = col0 + c + 4 * k4;
+                if (colv + 3 < p.b_rows) {
+                  st_global_v4f64(out + colv, acc[4 * k4], acc[4 * k4 + 1], acc[4 * k4 + 2], acc[4 * k4 + 3]);
+                } else {
+#pragma unroll
+                  for (int j = 0; j < 4; ++j)
+                    if (colv + j < p.b_rows) out[colv + j] = acc[4 * k4 + j];
+                }
+              }
+            }
           } else if (vec_ok) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
@@ -792,7 +824,7 @@ static int g_gemm_force_bk = 0;
 static int g_gemm_no_tp = 0;
 static int g_gemm_no_pair = 0;
 void set_gemm_debug_flags(int flags) {
-  g_gemm_dbg_flags = flags & 3;
+  g_gemm_dbg_flags = (flags & 3) | (((flags >> 23) & 1) << 2);  // bit 23: staged 16-byte epilogue accesses, no 256-bit ones
   g_gemm_no_pair = (flags >> 20) & 1;  // bit 20: no cta_group::2 pair tiles
   g_gemm_no_tp = (flags >> 3) & 1;  // bit 3: multi-pass through global read-modify-write instead of TMEM
   const int f = (flags >> 8) & 0xFF;  // bits 8..15: force the K-block width (32, 64, 128; 0 = auto)
