@@ -23,8 +23,14 @@
 namespace dfe {
 
 constexpr int kMaxStages = 8;
-constexpr int kGemmThreads = 320;  // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue (two per TMEM lane quarter)
-constexpr int kSmemLimit = 232448 - 13312;  // 227 KB minus the static shared memory (barriers, epilogue staging)
+#ifndef DFE_EPI_PER_QUARTER
+#define DFE_EPI_PER_QUARTER 2
+#endif
+constexpr int kEpiPerQuarter = DFE_EPI_PER_QUARTER;  // epilogue warps per TMEM lane quarter
+constexpr int kEpiWarps = 4 * kEpiPerQuarter;
+constexpr int kGemmThreads = 64 + 32 * kEpiWarps;  // warp 0 TMA, warp 1 MMA, warps 2.. epilogue
+// 227 KB minus the static shared memory (barriers, epilogue staging, column scales)
+constexpr int kSmemLimit = 232448 - (kEpiWarps * 1280 + 2048 + 512);
 
 struct GemmKernelParams {
   CUtensorMap mapA;
@@ -147,7 +153,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
   __shared__ __align__(8) uint64_t tmem_full_bar;
   __shared__ __align__(8) uint64_t tmem_empty_bar;
   __shared__ uint32_t tmem_slot;
-  __shared__ __align__(16) double epi_stage[8][16][10];  // per epilogue warp: 16 rows x 8 cols, 80 B pitch
+  __shared__ __align__(16) double epi_stage[kEpiWarps][16][10];  // per epilogue warp: 16 rows x 8 cols, 80 B pitch
   __shared__ int eb_sh[2][256];  // scale indices of the tile's columns (double buffered over tiles)
 
   const int warp = threadIdx.x >> 5;
@@ -170,7 +176,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
       mbar_init(&empty_bar[i], CL == 2 ? 2 : 1);
     }
     mbar_init(&tmem_full_bar, 1);
-    mbar_init(&tmem_empty_bar, CL == 4 ? 16 : kGemmThreads - 64);  // pair: one arrival per epilogue warp of both CTAs
+    mbar_init(&tmem_empty_bar, CL == 4 ? 2 * kEpiWarps : kGemmThreads - 64);  // pair: one arrival per epilogue warp of both CTAs
     fence_barrier_init();
   }
   if (warp == 1) {
@@ -347,8 +353,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     {
       const int et = (warp - 2) * 32 + lane;
       const long long col = (long long)tn * p.n_tile + et;
-      ebs[et] = (p.mode != kEpiInt32 && et < p.n_tile && col < p.b_rows) ? p.eB[z * p.eb_stride + col] : 0;
-      asm volatile("bar.sync 1, 256;" ::: "memory");  // epilogue warps only; buffer tile_no & 1 is free again
+      if (et < 256)
+        ebs[et] = (p.mode != kEpiInt32 && et < p.n_tile && col < p.b_rows) ? p.eB[z * p.eb_stride + col] : 0;
+      asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");  // epilogue warps only; buffer tile_no & 1 is free again
     }                                                  // once every warp has passed the next tile's barrier
     const int row_local = quarter * 32 + lane;
     const long long row = (long long)tm * kTileM + row_local;
@@ -397,7 +404,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         const bool last = (ch == chunk_hi - 1) && (ps == npass - 1);
         mbar_wait(&tmem_full_bar, iter & 1u);
         tc_fence_after();
-        for (int c = chalf * 16; c < p.n_tile; c += 32) {
+        for (int c = chalf * 16; c < p.n_tile; c += 16 * kEpiPerQuarter) {
           uint32_t v[16];
           if (p.mode == kEpiInt32) {
             for (int w = w_hi; w >= w_lo; --w) {
@@ -844,15 +851,15 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   if (bk == 0) {
     // widest swizzle span that still gives two stages (measured: 128-byte K blocks with two stages
     // beat 64-byte blocks with four: full 128-byte lines per TMA row and half the barrier traffic)
-    auto stages = [&](int cand) { return (kSmemLimit - 2048) / (int)stage_stride_for(s, nb, cand); };
+    auto stages = [&](int cand) { return (kSmemLimit - 1024) / (int)stage_stride_for(s, nb, cand); };
     if (stages(128) >= 2) bk = 128;
     else if (stages(64) >= 2) bk = 64;
     else bk = 32;
   }
   // a forced K-block width that leaves no room for even one stage is narrowed
-  while (bk > 32 && (kSmemLimit - 2048) / (int)stage_stride_for(s, nb, bk) < 1) bk /= 2;
+  while (bk > 32 && (kSmemLimit - 1024) / (int)stage_stride_for(s, nb, bk) < 1) bk /= 2;
   p.stage_stride = stage_stride_for(s, nb, bk);
-  p.num_stages = (int)((kSmemLimit - 2048) / p.stage_stride);
+  p.num_stages = (int)((kSmemLimit - 1024) / p.stage_stride);
   if (p.num_stages > kMaxStages) p.num_stages = kMaxStages;
   if (p.num_stages < 1) return cudaErrorInvalidValue;
   if (!make_plane_map(&p.mapA, g.A, g.k, g.a_rows, s, g.a_pitch, g.a_plane_stride, bk, kTileM) ||

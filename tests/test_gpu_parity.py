@@ -131,7 +131,9 @@ def test_weight_sums_flush_chunks(dfe, gpu_ws, s, k):
             assert np.array_equal(got[w - 2], ref[w]), f"chunk {ch} w={w}"
 
 
-@pytest.mark.parametrize("m,n,k", [(256, 256, 256), (300, 200, 1000), (128, 48, 4096), (1, 1, 1), (5, 700, 33)])
+# n % 4 == 0: 256-bit epilogue accesses; n = 250: 16-byte staged path; odd n: scalar path
+@pytest.mark.parametrize("m,n,k", [(256, 256, 256), (300, 200, 1000), (128, 48, 4096), (1, 1, 1), (5, 700, 33),
+                                   (200, 250, 520), (37, 131, 200)])
 def test_emul_gemm_matches_oracle_emulation_bitwise(dfe, gpu_ws, m, n, k):
     A, B = G.make_gemm_inputs(m, n, k, seed=3)
     Ad, Bd = dev(A), dev(B)
@@ -557,11 +559,12 @@ def test_jk_largest_config4_sampled(dfe, gpu_ws):
     assert np.sum(D * Kh) >= 0.0
 
 
-@pytest.mark.parametrize("flags", [8, 1 << 20, (1 << 20) | 8, 32 << 8, 64 << 8, 128 << 8])
+@pytest.mark.parametrize("flags", [8, 1 << 20, (1 << 20) | 8, 32 << 8, 64 << 8, 128 << 8, 1 << 23, (1 << 23) | 8])
 def test_emul_gemm_alternative_paths_bitwise(dfe, gpu_ws, flags):
     """The code paths the library does not pick by itself at these sizes (global read-modify-write
-    of multi-pass tiles, one CTA per tile instead of cta_group::2 pairs, every K-block width) must
-    give the same bits as the oracle's emulation."""
+    of multi-pass tiles, one CTA per tile instead of cta_group::2 pairs, every K-block width, the
+    staged 16-byte epilogue instead of 256-bit accesses) must give the same bits as the oracle's
+    emulation."""
     m, n, k = 300, 260, 1500
     A, B = G.make_gemm_inputs(m, n, k, seed=31)
     Ad, Bd = dev(A), dev(B)
@@ -576,7 +579,7 @@ def test_emul_gemm_alternative_paths_bitwise(dfe, gpu_ws, flags):
         dfe.lib.df_debug_set_gemm_flags(0)
 
 
-@pytest.mark.parametrize("flags", [4, 64, 4 | 8, 1 << 22, (1 << 22) | 64])
+@pytest.mark.parametrize("flags", [4, 64, 4 | 8, 1 << 22, (1 << 22) | 64, 1 << 23, (1 << 23) | 4 | 8])
 def test_jk_alternative_gemm5_paths(dfe, gpu_ws, flags):
     """GEMM(5) with one N tile (multi-pass), with the N halves on multicast CTA pairs instead of MMA
     pairs (bit 22), and with the halves on single CTAs (bit 6)."""
