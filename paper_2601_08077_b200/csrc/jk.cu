@@ -222,10 +222,13 @@ __global__ void __launch_bounds__(256) jk_j_gemv_kernel(const double* __restrict
 // (a warp instruction reads one 256-byte run of a packed row), converts them with the scale of
 // (q, R), and writes 16 bytes per plane into the staging tile [plane][q][128 + 16 pad]; after one
 // barrier (the tile is double buffered) the warps copy it out, 8 lanes per 128-byte line of
-// (plane, q, R).  Blocks are ordered [128 x 128 super-tile pair (A >= B)][q chunk][sub]: the first
+// (plane, q, R).  Blocks are ordered [q chunk][128 x 128 super-tile pair (A >= B)][sub]: the first
 // half of the subs are the row groups of the (A, B) block (rows in A, columns in B), the second
 // half those of the mirrored (B, A) block; both read the same 128 x 128 packed rows of this q
-// chunk (4 MB) back to back, so the second read is an L2 hit.  Two rows per block keep the number
+// chunk (4 MB) back to back, so the second read is an L2 hit.  The q chunk is the slowest index:
+// all lines written in a stretch of time then fall into the 32 q x nao rows of one chunk (49 MB
+// per plane), which the L2 write-back turns into longer DRAM bursts than with the tile pair
+// slowest (10.7 -> 10.1 ms at s = 4, 15.4 -> 14.3 ms at s = 6; groups of 2, 4, 8 chunks lie between).  Two rows per block keep the number
 // of tiles in flight, and with it the L2 working set, small (8 rows: 11.2 / 16.9 ms at s = 4 / 6
 // against 10.5 / 14.3 ms).  Four resident blocks per SM up to s = 4, three above (measured both ways).
 constexpr int kUnpackRows = 2;
@@ -241,8 +244,9 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
   int A, B;
   bool lower;
   const int sub = (int)(blockIdx.x % (2 * kSubs));
-  const int chunk = (int)(blockIdx.x / (2 * kSubs));
-  if (!tile_of_block(blockIdx.y, sub / kSubs, A, B, lower)) return;  // (A, B) = (row block, column block)
+  const int chunk = (int)blockIdx.y;
+  const unsigned tpair = blockIdx.x / (2 * kSubs);
+  if (!tile_of_block(tpair, sub / kSubs, A, B, lower)) return;  // (A, B) = (row block, column block)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int qg = q0 + chunk * 32 + lane;
   const bool q_ok = qg < q1;
@@ -456,7 +460,7 @@ cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, 
                                    int* status, cudaStream_t st) {
   const unsigned T128 = (unsigned)((nao + 127) / 128);
   if (pitch % 128 != 0 || pitch < 128 * (int64_t)T128) return cudaErrorInvalidValue;
-  dim3 grid((unsigned)(2 * (128 / kUnpackRows)) * (unsigned)((q1 - q0 + 31) / 32), T128 * (T128 + 1) / 2);
+  dim3 grid((unsigned)(2 * (128 / kUnpackRows)) * (T128 * (T128 + 1) / 2), (unsigned)((q1 - q0 + 31) / 32));
   const int smem = 2 * s * 32 * kUnpackPitch;
   cudaError_t err = cudaSuccess;
   DFE_DISPATCH_S(s, (err = unpack_split_s<SS>(grid, smem, st, Bp, nao, naux, q0, q1, emax, e5, planes5, pitch,
