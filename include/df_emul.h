@@ -197,7 +197,8 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
  *   bits 8-15  force the K-block width in bytes (32, 64, 128) bits 16-19 MMA probe: operand tiles
  *   bit 20     no cta_group::2 pair tiles                            walked (2 bits), swizzle (2 bits)
  *   bit 22     GEMM(5) N halves on multicast CTA pairs, never on MMA pairs
- *   bit 23     GEMM epilogue moves FP64 through the staged 16-byte path, never 256-bit accesses */
+ *   bit 23     GEMM epilogue moves FP64 through the staged 16-byte path, never 256-bit accesses
+ *   bit 24     df_emul_gemm keeps 128-column tiles at s <= 3 (default: 256 columns at s <= 2, 160 at s = 3) */
 int df_debug_set_gemm_flags(int flags);
 
 /* Number of GPU kernels this library has launched in this process. */

@@ -22,6 +22,7 @@ static int g_mode = DF_MODE_GUARDED;
 static int g_device_ok = -1;
 static int g_g5_split_n = 1;
 static int g_g5_cluster = 1;
+static int g_wide_n = 1;
 static int g_g5_pair_halves = 1;
 
 // ---- optional per-kernel-class CUDA-event timing (df_profile_*; bench.py's roofline) ----
@@ -164,7 +165,9 @@ static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m
   g.a_plane_stride = m * w.pitch;
   g.b_plane_stride = n * w.pitch;
   g.s = s;
-  g.n_tile = n > 128 ? 128 : pad16(n);
+  // 256-column tiles when all s accumulators still fit TMEM (s <= 2): one or three MMAs per K step
+  // are fed by 2 s plane tiles, so the operand feed, not the tensor pipe, bounds s = 1, 2
+  g.n_tile = n > 128 ? ((s <= 2 && n >= 256 && g_wide_n) ? 256 : (s == 3 && n >= 160 && g_wide_n) ? 160 : 128) : pad16(n);
   g.bk = 0;
   g.nz = 1;
   g.zk = nullptr;
@@ -670,7 +673,8 @@ int df_debug_set_gemm_flags(int flags) {
   set_gemm_debug_flags(flags);
   g_g5_split_n = (flags & 4) ? 0 : 1;  // bit 2: GEMM(5) keeps one N tile
   g_g5_cluster = (flags & 64) ? 0 : 1;  // bit 6: GEMM(5) N halves without the multicast pair
-  set_jk_debug_flags((flags >> 4) & 3);  // bits 4, 5: unpack kernel without stores / without loads
+  set_jk_debug_flags((flags >> 4) & 3);
+  g_wide_n = ((flags >> 24) & 1) ? 0 : 1;  // bit 24: df_emul_gemm never takes 256-column tiles  // bits 4, 5: unpack kernel without stores / without loads
   g_g5_pair_halves = ((flags >> 22) & 1) ? 0 : 1;  // bit 22: GEMM(5) N halves never on MMA pairs
   set_peak_tiles((flags >> 16) & 15);  // bits 16-19: MMA probe operand tiles / swizzle
   return DF_OK;

@@ -559,7 +559,7 @@ def test_jk_largest_config4_sampled(dfe, gpu_ws):
     assert np.sum(D * Kh) >= 0.0
 
 
-@pytest.mark.parametrize("flags", [8, 1 << 20, (1 << 20) | 8, 32 << 8, 64 << 8, 128 << 8, 1 << 23, (1 << 23) | 8])
+@pytest.mark.parametrize("flags", [8, 1 << 20, (1 << 20) | 8, 32 << 8, 64 << 8, 128 << 8, 1 << 23, (1 << 23) | 8, 1 << 24])
 def test_emul_gemm_alternative_paths_bitwise(dfe, gpu_ws, flags):
     """The code paths the library does not pick by itself at these sizes (global read-modify-write
     of multi-pass tiles, one CTA per tile instead of cta_group::2 pairs, every K-block width, the
@@ -570,7 +570,7 @@ def test_emul_gemm_alternative_paths_bitwise(dfe, gpu_ws, flags):
     Ad, Bd = dev(A), dev(B)
     dfe.lib.df_debug_set_gemm_flags(flags)
     try:
-        for s in (3, 6, 8):
+        for s in (1, 2, 3, 6, 8):  # s <= 2 takes 256-column tiles, s = 3 160-column tiles (bit 24: never)
             C = torch.empty((m, n), dtype=torch.float64, device=DEV)
             dfe.df_emul_gemm_slices(Ad, Bd, C, m, n, k, s)
             torch.cuda.synchronize()
