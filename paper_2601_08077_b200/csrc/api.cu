@@ -194,6 +194,7 @@ struct JkWs {
   double *rho, *rho_part;
   uint32_t* emax5;
   double* Jp;
+  double* jpart;  // [ceil(naux / 32)][npair] chunk partials of Eq. 4 (plain builds)
   uint32_t* cmaxC;
   int32_t* eC;
   int8_t* pc;
@@ -246,6 +247,7 @@ static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s,
   w.rho_part = c.take<double>(jk_rho_part_rows((int)nao) * naux);
   w.emax5 = planned ? nullptr : c.take<uint32_t>(nao * naux);
   w.Jp = c.take<double>(nao * (nao + 1) / 2);
+  w.jpart = planned ? nullptr : c.take<double>(((naux + 31) / 32) * (nao * (nao + 1) / 2));
   w.cmaxC = c.take<uint32_t>(w.a_pad);
   w.eC = c.take<int32_t>(w.a_pad);
   w.pc = c.take<int8_t>((int64_t)s * w.a_pad * w.pitchj);
@@ -314,11 +316,11 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     ProfScope ps(kPPassA, st);
     DFE_CK(launch_jk_pass_a(Bp, (int)nao, (int)naux, D, w.rho_part, w.rho, w.emax5, st));
   }
-  {
+  if (planned) {
     ProfScope ps(kPJGemv, st);
     DFE_CK(launch_jk_j_gemv(Bp, npair, (int)naux, w.rho, w.Jp, st));
     DFE_CK(launch_jk_j_unpack(w.Jp, (int)nao, J, st));
-  }
+  }  // a plain build sums Eq. 4 inside the unpack pass (chunk partials) and reduces them after it
 
   // ---- right operand of GEMM(5): C_occ columns -> K-major planes, a_pad rows (padding rows 0) ----
   DFE_CK(cudaMemsetAsync(w.eC, 0, sizeof(int32_t) * w.a_pad, st));
@@ -347,7 +349,13 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     if (!planned) {
       ProfScope ps(kPUnpack, st);
       DFE_CK(launch_jk_unpack_split(Bp, (int)nao, (int)naux, (int)qs0, (int)qs1, w.emax5, s, w.e5, w.p5,
-                                    w.pitchj, (int64_t)nq * nao * w.pitchj, w.status, st));
+                                    w.pitchj, (int64_t)nq * nao * w.pitchj, w.status, w.rho,
+                                    w.jpart + (qs0 / 32) * npair, st));
+    }
+    if (!planned && qs1 == naux) {
+      ProfScope ps(kPJGemv, st);
+      DFE_CK(launch_jk_j_reduce(w.jpart, (int)((naux + 31) / 32), npair, w.Jp, st));
+      DFE_CK(launch_jk_j_unpack(w.Jp, (int)nao, J, st));
     }
     // GEMM(5): X[i][q][a] = sum_j B^q_ij C_ja   (Eq. 5 / Eq. 12)
     GemmProblem g5 = {};
@@ -564,7 +572,7 @@ int df_jk_plan_create(const double* B_packed, int64_t nao, int64_t naux, int sma
     if (launch_jk_unpack_split(B_packed, (int)nao, (int)naux, 0, (int)naux, emax, smax,
                                reinterpret_cast<int32_t*>(pb + L.e5_off),
                                reinterpret_cast<int8_t*>(pb + L.planes_off), L.pitch, L.plane_stride,
-                               (int*)g_ws, st) != cudaSuccess)
+                               (int*)g_ws, nullptr, nullptr, st) != cudaSuccess)
       return DF_ERR_CUDA;
   }
   return DF_OK;

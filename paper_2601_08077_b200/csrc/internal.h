@@ -86,7 +86,9 @@ cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const do
 // unpack + split q in [q0, q1): planes5[t][(q - q0) * nao + i][pitch], e5[(q - q0) * nao + i]
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
-                                   int* status, cudaStream_t st);
+                                   int* status, const double* rho, double* jpart, cudaStream_t st);
+// jpart (may be null): [chunk of 32 q, counted from q0][npair] partials of Eq. 4; J_p = their sum in order
+cudaError_t launch_jk_j_reduce(const double* jpart, int nchunks, int64_t npair, double* Jp, cudaStream_t st);
 // X[(q, i)][a_pad] -> planes6[t][i][q * a_pad + a] (pitch6), e6[g][i] from xmax; qgroup[q] = group of q.
 // planes6 bytes past nq * a_pad in a row are never read (TMA extent).
 cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int s, int ng, const int* qgroup,

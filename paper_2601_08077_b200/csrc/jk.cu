@@ -3,7 +3,8 @@
 //
 //   jk_pass_a        rho_q = sum_ij B^q_ij D_ij (Eq. 3) fused with the row maxima
 //                    max_j |B^q_ij| that GEMM(5)'s left-operand scales need (R5)
-//   jk_j_gemv        J_p = sum_q B[p,q] rho_q   (Eq. 4), plain FP64
+//   jk_j_gemv        J_p = sum_q B[p,q] rho_q   (Eq. 4), plain FP64; a plain
+//                    build takes the chunk partials from the unpack pass instead (jk_j_reduce)
 //   jk_unpack_split  packed-symmetric B -> dense rows (q,i) x j as INT8 digit planes
 //                    ("symmetrise block to dense", fused with the split)
 //   jk_split_x       X (GEMM(5) output) -> digit planes with one scale per (i, q-group)
@@ -202,17 +203,88 @@ __global__ void __launch_bounds__(256) jk_rho_reduce_kernel(const double* __rest
   }
 }
 
+// J (Eq. 4) is summed the same way on both routes, so that a planned build and a plain build
+// give the same bits: J_p = sum over the 32-q chunks c, in increasing c, of the chunk's partial
+// sum_{q in c} B[p,q] rho_q, and the partial is the butterfly over the 32 lanes (lane = q within the
+// chunk; partners at distance 16, 8, 4, 2, 1; products rounded before the additions).
+//
+// tree4: four such butterflies at once.  Lane q holds y0..y3 = its terms of four packed rows; after
+// the first two levels a lane carries only one of the four sums (rows are handed over instead of
+// duplicated: 6 shuffles and 6 additions instead of 20), and every lane returns the complete sum
+// of row v = 2 * (lane bit 4) + (lane bit 3).  Additions commute bit for bit, so each row's result
+// equals the plain butterfly's.
+__device__ __forceinline__ double shfl_xor_f64(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+__device__ __forceinline__ double tree4(double y0, double y1, double y2, double y3, int lane) {
+  const bool b4 = (lane & 16) != 0, b3 = (lane & 8) != 0;
+  double k0 = b4 ? y2 : y0, k1 = b4 ? y3 : y1;
+  const double s0 = b4 ? y0 : y2, s1 = b4 ? y1 : y3;
+  k0 += shfl_xor_f64(s0, 16);
+  k1 += shfl_xor_f64(s1, 16);
+  double k = b3 ? k1 : k0;
+  const double sd = b3 ? k0 : k1;
+  k += shfl_xor_f64(sd, 8);
+  k += shfl_xor_f64(k, 4);
+  k += shfl_xor_f64(k, 2);
+  k += shfl_xor_f64(k, 1);
+  return k;
+}
+
+// Planned builds (no unpack pass to ride on): a warp owns four consecutive packed rows and walks
+// the chunks; sixteen loads of B per lane are in flight.
 __global__ void __launch_bounds__(256) jk_j_gemv_kernel(const double* __restrict__ Bp, long long npair, int naux,
                                                         const double* __restrict__ rho, double* __restrict__ Jp) {
   const int lane = threadIdx.x & 31;
-  const long long p = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
-  if (p >= npair) return;
-  const double* b = Bp + p * naux;
-  double acc = 0.0;
-  for (int q = lane; q < naux; q += 32) acc = fma(__ldg(b + q), __ldg(rho + q), acc);
+  const long long p0 = ((long long)blockIdx.x * 8 + (threadIdx.x >> 5)) * 4;
+  if (p0 >= npair) return;
+  const double* b[4];
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-  if (lane == 0) Jp[p] = acc;
+  for (int r = 0; r < 4; ++r) b[r] = Bp + (p0 + r < npair ? p0 + r : npair - 1) * naux;
+  const int nchunks = (naux + 31) >> 5;
+  double acc = 0.0;
+  int c = 0;
+  for (; c + 4 <= nchunks; c += 4) {
+    double x[4][4], rq[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int q = (c + u) * 32 + lane;
+      const bool ok = q < naux;
+      rq[u] = ok ? __ldg(rho + q) : 0.0;
+#pragma unroll
+      for (int r = 0; r < 4; ++r) x[u][r] = ok ? __ldg(b[r] + q) : 0.0;
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) acc += tree4(x[u][0] * rq[u], x[u][1] * rq[u], x[u][2] * rq[u], x[u][3] * rq[u], lane);
+  }
+  for (; c < nchunks; ++c) {
+    const int q = c * 32 + lane;
+    const bool ok = q < naux;
+    const double rq = ok ? __ldg(rho + q) : 0.0;
+    double x[4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) x[r] = ok ? __ldg(b[r] + q) : 0.0;
+    acc += tree4(x[0] * rq, x[1] * rq, x[2] * rq, x[3] * rq, lane);
+  }
+  const int v = ((lane >> 4) & 1) * 2 + ((lane >> 3) & 1);
+  if ((lane & 7) == 0 && p0 + v < npair) Jp[p0 + v] = acc;
+}
+
+// Plain builds: the unpack pass leaves one partial per (chunk, packed row) in jpart; J_p is their
+// sum in increasing chunk order.
+__global__ void __launch_bounds__(256) jk_j_reduce_kernel(const double* __restrict__ jpart, int nchunks,
+                                                          long long npair, double* __restrict__ Jp) {
+  const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= npair) return;
+  double acc = 0.0;
+  int c = 0;
+  for (; c + 8 <= nchunks; c += 8) {
+    double v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = __ldg(jpart + (long long)(c + u) * npair + p);
+#pragma unroll
+    for (int u = 0; u < 8; ++u) acc += v[u];
+  }
+  for (; c < nchunks; ++c) acc += __ldg(jpart + (long long)c * npair + p);
+  Jp[p] = acc;
 }
 
 // Unpack + split.  Output planes[t][(q, R)][C] want C-contiguous 128-byte lines, the input wants
@@ -238,7 +310,9 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
                                                               int q0, int q1, const uint32_t* __restrict__ emax,
                                                               int32_t* __restrict__ e5, int8_t* __restrict__ planes,
                                                               long long pitch, long long plane_stride,
-                                                              int* __restrict__ status, int dbg) {
+                                                              int* __restrict__ status, int dbg,
+                                                              const double* __restrict__ rho,
+                                                              double* __restrict__ jpart, long long npair) {
   extern __shared__ __align__(16) uint8_t ubuf[];  // [2][S][32][kUnpackPitch]
   constexpr int kSubs = 128 / kUnpackRows;
   int A, B;
@@ -258,6 +332,10 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
   const int kind = (A > B) ? 0 : (A < B) ? 1 : 2;
   const bool full = B * 128 + 128 <= nao;
   const int nq_blk = min(32, q1 - (q0 + chunk * 32));
+  // Eq. 4 rides on the lower blocks: they hold every packed element of this q chunk exactly once
+  const bool do_j = jpart != nullptr && lower;
+  const double rq = (do_j && q_ok) ? __ldg(rho + qg) : 0.0;
+  double* const jp_chunk = do_j ? jpart + (long long)chunk * npair : nullptr;
 #pragma unroll 1
   for (int r = 0; r < kUnpackRows; ++r) {
     const int R = A * 128 + (sub % kSubs) * kUnpackRows + r;
@@ -281,6 +359,18 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
     } else {
       if (kind == 1) load_row16<1, false>(x, bq, naux8, R, Cs, nao);
       else load_row16<2, false>(x, bq, naux8, R, Cs, nao);  // kind 0 has B < A: always full
+    }
+    if (do_j) {
+      // partial of J_p over this chunk's 32 q for the 16 packed rows p(R, Cs .. Cs + 15): lanes
+      // 0, 8, 16, 24 end up with the sums of columns 4 g4 + 0 .. 3 (tree4)
+      const int v = ((lane >> 4) & 1) * 2 + ((lane >> 3) & 1);
+#pragma unroll
+      for (int g4 = 0; g4 < 4; ++g4) {
+        const double k = tree4(x[4 * g4] * rq, x[4 * g4 + 1] * rq, x[4 * g4 + 2] * rq, x[4 * g4 + 3] * rq, lane);
+        const int C = Cs + 4 * g4 + v;
+        if ((lane & 7) == 0 && C <= R)  // C <= R < nao; a diagonal tile holds the rest as mirrors
+          jp_chunk[(long long)R * (R + 1) / 2 + C] = k;
+      }
     }
     uint32_t w[S][4];
 #pragma unroll
@@ -422,7 +512,13 @@ cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* 
 
 cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const double* rho, double* Jp,
                              cudaStream_t st) {
-  jk_j_gemv_kernel<<<(unsigned)((npair + 7) / 8), 256, 0, st>>>(Bp, npair, naux, rho, Jp);
+  jk_j_gemv_kernel<<<(unsigned)((npair + 31) / 32), 256, 0, st>>>(Bp, npair, naux, rho, Jp);
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_jk_j_reduce(const double* jpart, int nchunks, int64_t npair, double* Jp, cudaStream_t st) {
+  jk_j_reduce_kernel<<<(unsigned)((npair + 255) / 256), 256, 0, st>>>(jpart, nchunks, npair, Jp);
   count_launch();
   return cudaGetLastError();
 }
@@ -442,7 +538,8 @@ cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const do
 template <int S>
 static cudaError_t unpack_split_s(dim3 grid, int smem, cudaStream_t st, const double* Bp, int nao, int naux, int q0,
                                   int q1, const uint32_t* emax, int32_t* e5, int8_t* planes5, int64_t pitch,
-                                  int64_t plane_stride, int* status) {
+                                  int64_t plane_stride, int* status, const double* rho, double* jpart,
+                                  long long npair) {
   static bool attr_set = false;  // one opt-in per instantiation (s >= 6 stages more than 48 KB)
   if (!attr_set) {
     cudaError_t err = cudaFuncSetAttribute(jk_unpack_split_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -451,20 +548,20 @@ static cudaError_t unpack_split_s(dim3 grid, int smem, cudaStream_t st, const do
     attr_set = true;
   }
   jk_unpack_split_kernel<S><<<grid, 256, smem, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5, pitch, plane_stride,
-                                                     status, g_jk_dbg);
+                                                     status, g_jk_dbg, rho, jpart, npair);
   return cudaSuccess;
 }
 
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
-                                   int* status, cudaStream_t st) {
+                                   int* status, const double* rho, double* jpart, cudaStream_t st) {
   const unsigned T128 = (unsigned)((nao + 127) / 128);
   if (pitch % 128 != 0 || pitch < 128 * (int64_t)T128) return cudaErrorInvalidValue;
   dim3 grid((unsigned)(2 * (128 / kUnpackRows)) * (T128 * (T128 + 1) / 2), (unsigned)((q1 - q0 + 31) / 32));
   const int smem = 2 * s * 32 * kUnpackPitch;
   cudaError_t err = cudaSuccess;
   DFE_DISPATCH_S(s, (err = unpack_split_s<SS>(grid, smem, st, Bp, nao, naux, q0, q1, emax, e5, planes5, pitch,
-                                              plane_stride, status)));
+                                              plane_stride, status, rho, jpart, (long long)nao * (nao + 1) / 2)));
   if (err != cudaSuccess) return err;
   count_launch();
   return cudaGetLastError();
