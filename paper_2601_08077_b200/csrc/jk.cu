@@ -229,6 +229,25 @@ __device__ __forceinline__ double tree4(double y0, double y1, double y2, double 
   return k;
 }
 
+// tree16: the same for sixteen rows (x[i] = this lane's element of row i, rq = its rho): 16 shuffles and
+// additions for sixteen butterflies; lane 2 i (and 2 i + 1) returns the complete sum of row i.
+__device__ __forceinline__ double tree16(const double (&x)[16], double rq, int lane) {
+  const bool b4 = (lane & 16) != 0, b3 = (lane & 8) != 0, b2 = (lane & 4) != 0, b1 = (lane & 2) != 0;
+  double k8[8], k4[4], k2[2];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const double lo = x[i] * rq, hi = x[8 + i] * rq;
+    k8[i] = (b4 ? hi : lo) + shfl_xor_f64(b4 ? lo : hi, 16);
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) k4[i] = (b3 ? k8[4 + i] : k8[i]) + shfl_xor_f64(b3 ? k8[i] : k8[4 + i], 8);
+#pragma unroll
+  for (int i = 0; i < 2; ++i) k2[i] = (b2 ? k4[2 + i] : k4[i]) + shfl_xor_f64(b2 ? k4[i] : k4[2 + i], 4);
+  double k = (b1 ? k2[1] : k2[0]) + shfl_xor_f64(b1 ? k2[0] : k2[1], 2);
+  k += shfl_xor_f64(k, 1);
+  return k;
+}
+
 // Planned builds (no unpack pass to ride on): a warp owns four consecutive packed rows and walks
 // the chunks; sixteen loads of B per lane are in flight.
 __global__ void __launch_bounds__(256) jk_j_gemv_kernel(const double* __restrict__ Bp, long long npair, int naux,
@@ -361,16 +380,12 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
       else load_row16<2, false>(x, bq, naux8, R, Cs, nao);  // kind 0 has B < A: always full
     }
     if (do_j) {
-      // partial of J_p over this chunk's 32 q for the 16 packed rows p(R, Cs .. Cs + 15): lanes
-      // 0, 8, 16, 24 end up with the sums of columns 4 g4 + 0 .. 3 (tree4)
-      const int v = ((lane >> 4) & 1) * 2 + ((lane >> 3) & 1);
-#pragma unroll
-      for (int g4 = 0; g4 < 4; ++g4) {
-        const double k = tree4(x[4 * g4] * rq, x[4 * g4 + 1] * rq, x[4 * g4 + 2] * rq, x[4 * g4 + 3] * rq, lane);
-        const int C = Cs + 4 * g4 + v;
-        if ((lane & 7) == 0 && C <= R)  // C <= R < nao; a diagonal tile holds the rest as mirrors
-          jp_chunk[(long long)R * (R + 1) / 2 + C] = k;
-      }
+      // partial of J_p over this chunk's 32 q for the 16 packed rows p(R, Cs .. Cs + 15): lane 2 i
+      // ends up with the sum of column i (tree16), the even lanes store 128 contiguous bytes
+      const double k = tree16(x, rq, lane);
+      const int C = Cs + (lane >> 1);
+      if ((lane & 1) == 0 && C <= R)  // C <= R < nao; a diagonal tile holds the rest as mirrors
+        jp_chunk[(long long)R * (R + 1) / 2 + C] = k;
     }
     uint32_t w[S][4];
 #pragma unroll
