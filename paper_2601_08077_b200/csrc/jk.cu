@@ -76,7 +76,7 @@ __device__ __forceinline__ long long packed_row(int R, int C) {
 // per tile that re-read the same 256 KB through L2: 13 % of those reads missed (26.1 GB of DRAM
 // reads for 23.1 GB of B).  A plan (df_jk_plan_create) runs EMAX alone once, a planned build RHO alone.
 template <bool RHO, bool EMAX>
-__global__ void __launch_bounds__(256) jk_pass_a_kernel(const double* __restrict__ Bp, int nao, int naux,
+__global__ void __launch_bounds__(256, EMAX ? 4 : 5) jk_pass_a_kernel(const double* __restrict__ Bp, int nao, int naux,
                                                         const double* __restrict__ D,
                                                         double* __restrict__ rho_part,
                                                         uint32_t* __restrict__ emax) {
