@@ -350,8 +350,8 @@ def run_ours(args, cfg):
                      "launches": n5 + n6, "avg_launch_ms": (ms5 + ms6) / max(1, n5 + n6),
                      "share_of_step": (ms5 + ms6) / ms_total,
                      # dram__bytes_read+write per launch, ncu --set full at s = 4 (profiles/r01_ncu_summary.md):
-                     # GEMM(5) 32.4 GB, GEMM(6) 4.8 GB -> mean over the two launches of a build
-                     "traffic": 0.5 * (32.4e9 + 4.8e9), "traffic_unit": "bytes per launch (s = 4)"},
+                     # GEMM(5) 25.9 + 6.1 GB, GEMM(6) 4.5 + 0.2 GB -> mean over the two launches of a build
+                     "traffic": 0.5 * (32.0e9 + 4.7e9), "traffic_unit": "bytes per launch (s = 4)"},
         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items() if v[1]},
     }
     if planned is not None:
