@@ -9,10 +9,10 @@
 //       out  += 2^(eA_i + eB_j + 2 - 8 w) P^(w)    -- w descending, ONE running FP64 sum
 //
 // Structure: warp 0 = TMA producer (one lane), warp 1 = TMEM allocator + MMA issuer (one lane),
-// warps 2..5 = epilogue (TMEM lane quarter = warp % 4).  All s digit planes of a K block sit in
-// shared memory together, so 2 s plane tiles feed up to s(s+1)/2 MMAs (hard
-// part 4).  Operands are K-major INT8 planes; the K-block width BK equals the TMA/UMMA swizzle
-// span (32, 64 or 128 bytes) and is chosen so that at least three stages fit.
+// warps 2..9 = epilogue (TMEM lane quarter = warp % 4, two warps per quarter).  All s digit planes
+// of a K block sit in shared memory together, so 2 s plane tiles feed up to s(s+1)/2 MMAs (SURVEY
+// section 7, hard part 4).  Operands are K-major INT8 planes; the K-block width BK equals the
+// TMA/UMMA swizzle span (32, 64 or 128 bytes): the widest one that still leaves two stages.
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
