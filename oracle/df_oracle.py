@@ -338,15 +338,12 @@ def emul_gemm(A: np.ndarray, B: np.ndarray, s: int) -> np.ndarray:
 # ----------------------------------------------------------------------------
 
 
-def pad16(n: int) -> int:
-    return 16 * ((n + 15) // 16)
-
-
 def q_groups(naux: int, nocc: int, s: int, qblock: int = 512):
-    """Consecutive-q groups for GEMM(6) (reading R5): q is cut into blocks of
-    `qblock`; every block into runs of at most QG = floor(KFLUSH(s) / pad16(nocc))
-    consecutive q (so one group's contraction fits one INT32 chunk)."""
-    qg = max(1, kflush(s) // pad16(nocc))
+    """Consecutive-q groups for GEMM(6) (reading R5; "a run of
+    consecutive q with |g| nocc <= k_flush"): q is cut into blocks of `qblock`; every
+    block into runs of at most QG = floor(KFLUSH(s) / nocc) consecutive q, so that the
+    |g| nocc contraction elements of one group fit one INT32 chunk (step 6)."""
+    qg = max(1, kflush(s) // nocc)
     groups = []
     for b0 in range(0, naux, qblock):
         b1 = min(naux, b0 + qblock)

@@ -187,8 +187,6 @@ static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m
 // ---------------------------------------------------------------------------
 // df_jk_build
 // ---------------------------------------------------------------------------
-constexpr int kQBlock = 512;  // BASELINE.json config 4: "naux blocks of 512"
-
 struct JkWs {
   int* status;
   double *rho, *rho_part;
@@ -201,13 +199,14 @@ struct JkWs {
   int32_t* e5;
   int8_t* p5;
   double* X;
-  int *qgroup, *gcol;
+  int *qgroup, *qcol, *gcol;
   uint32_t* xmax;
   int32_t* e6;
   int8_t* p6;
   double* Kpart;
   int64_t pitchj, pitch6, bytes;
-  int a_pad, QG, gpb, ngmax;
+  int a_pad, ngmax;
+  GroupGeom gg;
 };
 
 // Plan buffer (df_jk_plan_create): everything about B that does not change over an SCF.
@@ -234,14 +233,13 @@ static PlanLayout plan_layout(int64_t nao, int64_t naux, int smax) {
 static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s, int64_t QS, bool planned = false) {
   Carver c(base);
   JkWs w;
-  w.a_pad = pad16(nocc);
-  w.QG = kflush_for(s) / w.a_pad;
-  if (w.QG < 1) w.QG = 1;
-  w.gpb = (kQBlock + w.QG - 1) / w.QG;
-  w.ngmax = (int)((QS + kQBlock - 1) / kQBlock) * w.gpb;
+  w.gg = group_geom(s, (int)nocc);
+  w.a_pad = w.gg.a_pad;
+  w.ngmax = group_count(w.gg, (int)QS);
   // rows of whole 128-byte lines: the unpack pass writes full lines (1.2 % of a build at config 3)
   w.pitchj = round_up(nao, 128);
-  w.pitch6 = plane_pitch(QS * w.a_pad);
+  // every q-group starts at a multiple of 32 columns: at most 16 zero columns after each group
+  w.pitch6 = plane_pitch(QS * w.a_pad + 16 * (int64_t)w.ngmax);
   w.status = c.take<int>(64);
   w.rho = c.take<double>(naux);
   w.rho_part = c.take<double>(jk_rho_part_rows((int)nao) * naux);
@@ -255,6 +253,7 @@ static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s,
   w.p5 = planned ? nullptr : c.take<int8_t>((int64_t)s * QS * nao * w.pitchj);
   w.X = c.take<double>(nao * QS * w.a_pad);
   w.qgroup = c.take<int>(QS);
+  w.qcol = c.take<int>(QS);
   w.gcol = c.take<int>(w.ngmax + 1);
   w.xmax = c.take<uint32_t>((int64_t)w.ngmax * nao);
   w.e6 = c.take<int32_t>((int64_t)w.ngmax * nao);
@@ -264,15 +263,16 @@ static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s,
   return w;
 }
 
-// q-group tables of one super-block [qs0, qs1) (R5): q is cut into blocks of 512, every
-// block into runs of QG consecutive q.  qgroup[q - qs0] = local group id; gcol[g] = first X column
-// (= contraction offset of GEMM(6)) of group g; gcol[ng] = end.
-__global__ void jk_group_tables_kernel(int nq, int QG, int gpb, int a_pad, int ng, int* qgroup, int* gcol) {
-  for (int ql = threadIdx.x; ql < nq; ql += blockDim.x) qgroup[ql] = (ql / kQBlock) * gpb + (ql % kQBlock) / QG;
-  for (int g = threadIdx.x; g <= ng; g += blockDim.x) {
-    const int qstart = (g / gpb) * kQBlock + (g % gpb) * QG;
-    gcol[g] = (g == ng) ? nq * a_pad : qstart * a_pad;
+// q-group tables of one super-block of nq consecutive q (R5, internal.h GroupGeom):
+// qgroup[ql] = local group id, qcol[ql] = first planes6 column of q, gcol[g] = first column
+// (= contraction offset of GEMM(6)) of group g, a multiple of 32; gcol[ng] = the end.
+__global__ void jk_group_tables_kernel(int nq, GroupGeom gg, int ng, int* qgroup, int* qcol, int* gcol) {
+  for (int ql = threadIdx.x; ql < nq; ql += blockDim.x) {
+    const int g = (ql / kQBlock) * gg.gpb + (ql % kQBlock) / gg.QG;
+    qgroup[ql] = g;
+    qcol[ql] = group_col(gg, g, nq, ng) + (ql - group_q0(gg, g)) * gg.a_pad;
   }
+  for (int g = threadIdx.x; g <= ng; g += blockDim.x) gcol[g] = group_col(gg, g, nq, ng);
 }
 
 // plan != nullptr (with its slice count smax): a planned build, GEMM(5) reads the plan's planes.
@@ -335,12 +335,14 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
   for (int64_t qs0 = 0; qs0 < naux; qs0 += QS) {
     const int64_t qs1 = qs0 + QS < naux ? qs0 + QS : naux;
     const int nq = (int)(qs1 - qs0);
-    const int nfull = nq / kQBlock, rem = nq % kQBlock;
-    const int ng = nfull * w.gpb + (rem + w.QG - 1) / w.QG;
-    const int64_t ncol = (int64_t)nq * w.a_pad;
+    const int ng = group_count(w.gg, nq);
+    // contraction extent of GEMM(6): the padded columns of all groups (every group boundary is a
+    // multiple of 32, the K extent of one MMA: an MMA never straddles two groups)
+    const int64_t ncol = group_col(w.gg, ng, nq, ng);
     const int64_t pitch6 = plane_pitch(ncol);
+    if (ncol % 32 != 0 || pitch6 > w.pitch6) return DF_ERR_DIM;
 
-    jk_group_tables_kernel<<<1, 256, 0, st>>>(nq, w.QG, w.gpb, w.a_pad, ng, w.qgroup, w.gcol);
+    jk_group_tables_kernel<<<1, 256, 0, st>>>(nq, w.gg, ng, w.qgroup, w.qcol, w.gcol);
     count_launch();
     DFE_CK(cudaGetLastError());
     DFE_CK(cudaMemsetAsync(w.xmax, 0, sizeof(uint32_t) * ng * nao, st));
@@ -412,8 +414,8 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     // X -> planes6 with one scale per (i, group)
     {
       ProfScope ps(kPSplitX, st);
-      DFE_CK(launch_jk_split_x(w.X, (int)nao, nq, w.a_pad, s, ng, w.qgroup, w.xmax, w.e6, w.p6, pitch6,
-                               (int64_t)nao * pitch6, w.status, st));
+      DFE_CK(launch_jk_split_x(w.X, (int)nao, nq, w.a_pad, s, ng, w.qgroup, w.qcol, w.gcol, w.xmax, w.e6, w.p6,
+                               pitch6, (int64_t)nao * pitch6, w.status, st));
     }
     if (e6_out)
       DFE_CK(cudaMemcpyAsync(e6_out + (int64_t)gtotal * nao, w.e6, sizeof(int32_t) * ng * nao,

@@ -933,7 +933,9 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.a_rows = g.a_rows;
   p.b_rows = g.b_rows;
   p.k = (int)g.k;
-  p.kflush = kflush_for(s);
+  // a z item (q-group of GEMM(6)) is one flush chunk by construction: its contraction holds at most
+  // kflush(s) elements that are not zero padding (R5), whatever its padded extent
+  p.kflush = g.zk ? (1 << 30) : kflush_for(s);
   p.zk = g.zk;
   p.eA = g.eA;
   p.eB = g.eB;

@@ -14,6 +14,42 @@ inline int kflush_for(int s) { return 32 * (131071 / (32 * s)); }
 
 void count_launch(int n = 1);
 
+// q-groups of GEMM(6) (R5): q is cut into blocks of 512, every block into runs of
+// QG = floor(KFLUSH(s) / nocc) consecutive q (one group's |g| nocc contraction elements fit one INT32
+// chunk).  In planes6 a q owns a_pad = pad16(nocc) columns (the padding columns are zero digits) and
+// every group starts at a multiple of 32 columns -- the K extent of one MMA -- with zero bytes
+// between the end of a group and the start of the next, so no MMA ever straddles two groups.
+constexpr int kQBlock = 512;  // BASELINE.json config 4: "naux blocks of 512"
+struct GroupGeom {
+  int QG, gpb, a_pad;
+  int wfull;   // padded column width of a full group
+  int wblock;  // padded column width of a full 512-q block
+};
+inline GroupGeom group_geom(int s, int nocc) {
+  GroupGeom g;
+  g.a_pad = (int)round_up(nocc, 16);
+  g.QG = kflush_for(s) / nocc;
+  if (g.QG < 1) g.QG = 1;
+  if (g.QG > kQBlock) g.QG = kQBlock;
+  g.gpb = (kQBlock + g.QG - 1) / g.QG;
+  g.wfull = (int)round_up((int64_t)g.QG * g.a_pad, 32);
+  g.wblock = (g.gpb - 1) * g.wfull + (int)round_up((int64_t)(kQBlock - (g.gpb - 1) * g.QG) * g.a_pad, 32);
+  return g;
+}
+// number of groups of nq consecutive q (a super-block starts at a multiple of 512)
+inline int group_count(const GroupGeom& g, int nq) {
+  return (nq / kQBlock) * g.gpb + ((nq % kQBlock) + g.QG - 1) / g.QG;
+}
+// first q of group gi; first planes6 column of group gi (gi == ng: the end)
+__host__ __device__ inline int group_q0(const GroupGeom& g, int gi) { return (gi / g.gpb) * 512 + (gi % g.gpb) * g.QG; }
+__host__ __device__ inline int group_col(const GroupGeom& g, int gi, int nq, int ng) {
+  if (gi < ng) return (gi / g.gpb) * g.wblock + (gi % g.gpb) * g.wfull;
+  const int last = ng - 1;
+  const int q0 = (last / g.gpb) * 512 + (last % g.gpb) * g.QG;
+  const int w = (nq - q0) * g.a_pad;
+  return (last / g.gpb) * g.wblock + (last % g.gpb) * g.wfull + (w + 31) / 32 * 32;
+}
+
 // ---- split.cu -------------------------------------------------------------
 // rows x cols FP64 (leading dimension ld) -> e[rows], planes[t][rows][pitch].
 cudaError_t launch_split_rows(const double* X, int64_t rows, int64_t cols, int64_t ld, int s, int32_t* e,
@@ -38,9 +74,10 @@ struct GemmProblem {
   int s;                         // slices
   int n_tile;                    // output columns per CTA tile (multiple of 16, <= 256)
   int bk;                        // K-block bytes = swizzle span: 32, 64, 128 (0 = auto)
-  // z items (q-groups): item z contracts K range [zk[z], zk[z+1]) (device int array of nz+1), or
-  // the whole [0, k) when zk == nullptr (then nz must be 1).  Each z item is cut into flush
-  // chunks of kflush(s) contraction elements.
+  // z items (q-groups): item z contracts K range [zk[z], zk[z+1]) (device int array of nz+1; every
+  // entry a multiple of 32, the K extent of one MMA, and every item ONE flush chunk: at most
+  // kflush(s) of its contraction elements are not zero padding), or the whole [0, k) when
+  // zk == nullptr (then nz must be 1), cut into flush chunks of kflush(s) contraction elements.
   int nz;
   const int* zk;
   const int32_t* eA;  // scale indices, eA[z * ea_stride + row]
@@ -89,11 +126,14 @@ cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, 
                                    int* status, const double* rho, double* jpart, cudaStream_t st);
 // jpart (may be null): [chunk of 32 q, counted from q0][npair] partials of Eq. 4; J_p = their sum in order
 cudaError_t launch_jk_j_reduce(const double* jpart, int nchunks, int64_t npair, double* Jp, cudaStream_t st);
-// X[(q, i)][a_pad] -> planes6[t][i][q * a_pad + a] (pitch6), e6[g][i] from xmax; qgroup[q] = group of q.
-// planes6 bytes past nq * a_pad in a row are never read (TMA extent).
+// X[(q, i)][a_pad] -> planes6[t][i][qcol[q] + a] (pitch6), e6[g][i] from xmax; qgroup[q] = group of q,
+// qcol[q] = its first column, gcol[g] = first column of group g (gcol[ng] = the end; multiples of 32).
+// The gap between the last q of a group and the next group is filled with zero bytes; bytes past
+// gcol[ng] in a row are never read (TMA extent).
 cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int s, int ng, const int* qgroup,
-                              const uint32_t* xmax, int32_t* e6, int8_t* planes6, int64_t pitch6,
-                              int64_t plane_stride6, int* status, cudaStream_t st);
+                              const int* qcol, const int* gcol, const uint32_t* xmax, int32_t* e6,
+                              int8_t* planes6, int64_t pitch6, int64_t plane_stride6, int* status,
+                              cudaStream_t st);
 // K (+)= sum_g Kpart[g] over lower block-triangle tiles (tile = 128), mirrored.
 cudaError_t launch_jk_k_reduce(const double* Kpart, int ng, int nao, int accumulate, double* K,
                                cudaStream_t st);

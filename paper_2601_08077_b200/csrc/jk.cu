@@ -430,13 +430,16 @@ __global__ void jk_x_scale_kernel(const uint32_t* __restrict__ xmax, long long n
   if (stt) atomicOr(status, stt);
 }
 
-// X[(q, i)][a_pad] (GEMM(5)'s output, one contiguous 128-row block per tile) -> planes6[t][i][q * a_pad + a]
+// X[(q, i)][a_pad] (GEMM(5)'s output, one contiguous 128-row block per tile) -> planes6[t][i][qcol[q] + a]
 // with the scale of (i, group of q).  A block owns one i and 32 consecutive q: it reads 32 runs of
-// a_pad doubles and writes one contiguous run of 32 * a_pad bytes per plane; a thread converts 16
-// consecutive columns.
+// a_pad doubles and writes one contiguous run of 32 * a_pad bytes per plane (with a 16-byte gap of
+// zeros where a group ends off a multiple of 32 columns: every group of GEMM(6) starts on the K extent
+// of an MMA); a thread converts 16 consecutive columns.
 template <int S>
 __global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restrict__ X, int nao, int nq, int a_pad,
                                                          const int* __restrict__ qgroup,
+                                                         const int* __restrict__ qcol,
+                                                         const int* __restrict__ gcol,
                                                          const int32_t* __restrict__ e6,
                                                          int8_t* __restrict__ planes, long long pitch,
                                                          long long plane_stride) {
@@ -447,7 +450,8 @@ __global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restric
     const int ql = u / runs_per_q, run = u - ql * runs_per_q;
     const int q = blockIdx.x * 32 + ql;
     if (q >= nq) break;
-    const double scale = pow2_double(63 - e6[(long long)qgroup[q] * nao + i]);
+    const int g = qgroup[q];
+    const double scale = pow2_double(63 - e6[(long long)g * nao + i]);
     const double2* src = reinterpret_cast<const double2*>(X + ((long long)q * nao + i) * a_pad + run * 16);
     double2 v[8];
 #pragma unroll
@@ -467,10 +471,17 @@ __global__ void __launch_bounds__(256) jk_split_x_kernel(const double* __restric
       for (int t = 0; t < S; ++t)
         w[t][g4] = (t < 4) ? pack4_digit(hi[0], hi[1], hi[2], hi[3], 3 - t) : pack4_digit(lo[0], lo[1], lo[2], lo[3], 7 - t);
     }
+    const long long col = qcol[q];
+    int8_t* const dst = planes + (long long)i * pitch + col + run * 16;
 #pragma unroll
     for (int t = 0; t < S; ++t)
-      *reinterpret_cast<uint4*>(planes + t * plane_stride + (long long)i * pitch + (long long)q * a_pad + run * 16) =
-          make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+      *reinterpret_cast<uint4*>(dst + t * plane_stride) = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+    // the last q of a group whose end is not a multiple of 32 columns: zero digits up to the next group
+    if (run == runs_per_q - 1 && col + a_pad < gcol[g + 1] && (q + 1 == nq || qgroup[q + 1] != g)) {
+#pragma unroll
+      for (int t = 0; t < S; ++t)
+        *reinterpret_cast<uint4*>(dst + t * plane_stride + 16) = make_uint4(0u, 0u, 0u, 0u);
+    }
   }
 }
 
@@ -583,13 +594,14 @@ cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, 
 }
 
 cudaError_t launch_jk_split_x(const double* X, int nao, int nq, int a_pad, int s, int ng, const int* qgroup,
-                              const uint32_t* xmax, int32_t* e6, int8_t* planes6, int64_t pitch6,
-                              int64_t plane_stride6, int* status, cudaStream_t st) {
+                              const int* qcol, const int* gcol, const uint32_t* xmax, int32_t* e6,
+                              int8_t* planes6, int64_t pitch6, int64_t plane_stride6, int* status,
+                              cudaStream_t st) {
   const long long n = (long long)ng * nao;
   jk_x_scale_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(xmax, n, e6, status);
   dim3 grid((unsigned)((nq + 31) / 32), (unsigned)nao);
-  DFE_DISPATCH_S(s, (jk_split_x_kernel<SS><<<grid, 256, 0, st>>>(X, nao, nq, a_pad, qgroup, e6, planes6, pitch6,
-                                                                 plane_stride6)));
+  DFE_DISPATCH_S(s, (jk_split_x_kernel<SS><<<grid, 256, 0, st>>>(X, nao, nq, a_pad, qgroup, qcol, gcol, e6, planes6,
+                                                                 pitch6, plane_stride6)));
   count_launch(2);
   return cudaGetLastError();
 }

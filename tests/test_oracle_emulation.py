@@ -324,15 +324,27 @@ def test_max_slices_below_1e12_vs_plain():
 # ------------------------------------------------------------------ step 7 (K path)
 
 
-def test_q_groups_cover_and_fit():
-    for naux, nocc, s, qb in [(160, 10, 3, 512), (1700, 50, 8, 512), (4000, 150, 4, 512), (37, 250, 8, 16)]:
+def test_q_groups_rule_and_int32_guard():
+    """Reading R5 / SURVEY 8(c) step 7, stated without the oracle's formula: the groups partition
+    [0, naux) in order, never straddle a q-block, are as long as the INT32 guard allows, and the worst
+    case of one weight sum over a group (s pairs, every digit -128: s |g| nocc 2^14) stays below 2^31."""
+    for naux, nocc, s, qb in [(160, 10, 3, 512), (1700, 50, 8, 512), (4000, 150, 4, 512), (4000, 150, 6, 512),
+                              (6000, 250, 5, 512), (37, 250, 8, 16), (1300, 70, 4, 512), (700, 1, 1, 512)]:
         g = O.q_groups(naux, nocc, s, qb)
         assert g[0][0] == 0 and g[-1][1] == naux
         for (a0, a1), (b0, b1) in zip(g[:-1], g[1:]):
-            assert a1 == b0
+            assert a1 == b0 and a0 < a1
         for g0, g1 in g:
-            assert (g1 - g0) * O.pad16(nocc) <= O.kflush(s) or g1 - g0 == 1
+            n = g1 - g0
             assert g0 // qb == (g1 - 1) // qb  # never straddles a q-block
+            assert s * n * nocc * (1 << 14) < (1 << 31)  # INT32 guard, true worst case
+            last_of_block = g1 == naux or g1 % qb == 0
+            if not last_of_block:
+                # maximal: one more q would exceed the flush length (a multiple of the 32-byte MMA K)
+                k_allowed = 32 * (((1 << 17) - 1) // (32 * s))
+                assert (n + 1) * nocc > k_allowed
+    # the configuration the benchmark runs (PAPER.md:200-222 shapes): 512 = 218 + 218 + 76 at s = 4
+    assert O.q_groups(4000, 150, 4)[:3] == [(0, 218), (218, 436), (436, 512)]
 
 
 def test_k_path_exact_on_small_integers():
