@@ -13,7 +13,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdfemul.so")
-SOURCES = ["api.cu", "split.cu", "gemm_i8.cu", "jk.cu"]
+SOURCES = ["api.cu", "split.cu", "gemm_i8.cu", "jk.cu", "tmap.cu"]
 HEADERS = ["common.cuh", "internal.h", os.path.join("..", "..", "include", "df_emul.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -788,38 +788,13 @@ cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStrea
 // ---------------------------------------------------------------------------
 // host side: tensor maps and launch
 // ---------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static EncodeTiledFn get_encode_fn() {
-  static EncodeTiledFn fn = nullptr;
-  if (!fn) {
-    void* ptr = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
-      fn = (EncodeTiledFn)ptr;
-  }
-  return fn;
-}
-
 // planes [plane][rows][pitch] int8 -> 3-D map (k, rows, plane), box (bk, box_rows, 1)
 static bool make_plane_map(CUtensorMap* map, const int8_t* base, int64_t k, int64_t rows, int planes,
                            int64_t pitch, int64_t plane_stride, int bk, int box_rows) {
-  EncodeTiledFn fn = get_encode_fn();
-  if (!fn) return false;
-  cuuint64_t dims[3] = {(cuuint64_t)k, (cuuint64_t)rows, (cuuint64_t)planes};
-  cuuint64_t strides[2] = {(cuuint64_t)pitch, (cuuint64_t)plane_stride};
-  cuuint32_t box[3] = {(cuuint32_t)bk, (cuuint32_t)box_rows, 1u};
-  cuuint32_t estr[3] = {1u, 1u, 1u};
-  const CUtensorMapSwizzle swz = bk == 128  ? CU_TENSOR_MAP_SWIZZLE_128B
-                                 : bk == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
-                                            : CU_TENSOR_MAP_SWIZZLE_32B;
-  CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void*)base, dims, strides, box, estr,
-                  CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS;
+  const uint64_t dims[3] = {(uint64_t)k, (uint64_t)rows, (uint64_t)planes};
+  const uint64_t strides[2] = {(uint64_t)pitch, (uint64_t)plane_stride};
+  const uint32_t box[3] = {(uint32_t)bk, (uint32_t)box_rows, 1u};
+  return encode_tensor_map(map, 0, 3, base, dims, strides, box, bk);
 }
 
 static uint32_t stage_stride_for(int s, int n_tile, int bk) {

@@ -50,6 +50,13 @@ __host__ __device__ inline int group_col(const GroupGeom& g, int gi, int nq, int
   return (last / g.gpb) * g.wblock + (last % g.gpb) * g.wfull + (w + 31) / 32 * 32;
 }
 
+// ---- tmap.cu ---------------------------------------------------------------
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked).
+// dtype: 0 = UINT8, 1 = FLOAT64; swizzle: 0 (none), 32, 64, 128 bytes.  dims/box: rank entries,
+// strides: rank - 1 entries in bytes (dimension 0 is contiguous).  map: a CUtensorMap (128 bytes).
+bool encode_tensor_map(void* map, int dtype, int rank, const void* base, const uint64_t* dims,
+                       const uint64_t* strides, const uint32_t* box, int swizzle);
+
 // ---- split.cu -------------------------------------------------------------
 // rows x cols FP64 (leading dimension ld) -> e[rows], planes[t][rows][pitch].
 cudaError_t launch_split_rows(const double* X, int64_t rows, int64_t cols, int64_t ld, int s, int32_t* e,

@@ -566,13 +566,10 @@ static cudaError_t unpack_split_s(dim3 grid, int smem, cudaStream_t st, const do
                                   int q1, const uint32_t* emax, int32_t* e5, int8_t* planes5, int64_t pitch,
                                   int64_t plane_stride, int* status, const double* rho, double* jpart,
                                   long long npair) {
-  static bool attr_set = false;  // one opt-in per instantiation (s >= 6 stages more than 48 KB)
-  if (!attr_set) {
-    cudaError_t err = cudaFuncSetAttribute(jk_unpack_split_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           2 * S * 32 * kUnpackPitch);
-    if (err != cudaSuccess) return err;
-    attr_set = true;
-  }
+  // set on every launch (s >= 6 stages more than 48 KB): the attribute is per device
+  cudaError_t err = cudaFuncSetAttribute(jk_unpack_split_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         2 * S * 32 * kUnpackPitch);
+  if (err != cudaSuccess) return err;
   jk_unpack_split_kernel<S><<<grid, 256, smem, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5, pitch, plane_stride,
                                                      status, g_jk_dbg, rho, jpart, npair);
   return cudaSuccess;

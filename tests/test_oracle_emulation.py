@@ -392,6 +392,30 @@ def test_k_path_max_slices():
     assert O.rel_frobenius(O.emul_df_k(Bp, cfg.nao, C, 8), K) <= 1e-12
 
 
+def test_level0_emulation_is_at_least_fp64_accurate():
+    """Table 1's level 0 is "standard FP64", relative accuracy 2.2e-16.  The library
+    has no native-FP64 GEMM: the caller-side schedule passes tol = 2^-52 and the guarded policy turns
+    that into s = 8.  Pin what that delivers against an extended-precision reference (x86 long double,
+    64-bit mantissa): on the config-1-like GEMM data and on the config-0 K path the s = 8 emulation is
+    closer to the exact result than the plain FP64 evaluation itself, and within 2.2e-16."""
+    assert O.slices_for_tol(2.0 ** -52, "guarded") == 8
+    A, B = make_gemm_inputs(96, 80, 640, seed=3)
+    ref = O.gemm_longdouble(A, B)
+    e_emul = O.rel_frobenius(O.emul_gemm(A, B, 8).astype(np.longdouble), ref)
+    e_fp64 = O.rel_frobenius(O.gemm_plain(A, B).astype(np.longdouble), ref)
+    assert e_emul <= e_fp64 and e_emul <= 2.0 ** -52, (e_emul, e_fp64)
+    cfg = CONFIGS["tiny"]
+    Bp, C, D = make_df_inputs(cfg)
+    Kl = np.zeros((cfg.nao, cfg.nao), dtype=np.longdouble)
+    Cl = C.astype(np.longdouble)
+    for q in range(cfg.naux):
+        Xq = O.unpack_sym(Bp[:, q], cfg.nao).astype(np.longdouble) @ Cl
+        Kl += Xq @ Xq.T
+    e_emul = O.rel_frobenius(O.emul_df_k(Bp, cfg.nao, C, 8).astype(np.longdouble), Kl)
+    e_fp64 = O.rel_frobenius(O.df_k(Bp, cfg.nao, C).astype(np.longdouble), Kl)
+    assert e_emul <= e_fp64 and e_emul <= 2.0 ** -52, (e_emul, e_fp64)
+
+
 def test_status_bits():
     X = np.ones((3, 4))
     assert O.operand_status(X) == 0

@@ -52,6 +52,75 @@ def _worker(rank, world, port, out):
     dist.destroy_process_group()
 
 
+def _oracle_build(calls, planned):
+    """Stand-in for the binding's build call in the CPU test (no GPU here): the per-shard partial J, K
+    come from the oracle, written into the caller's tensors exactly as df_jk_build does on a GPU."""
+    def build(*args):
+        if planned:
+            _plan, Bs, nao, naux, Cocc, nocc, D, tol, J, K, _stream = args
+        else:
+            Bs, nao, naux, Cocc, nocc, D, tol, J, K, _stream = args
+        calls.append(("planned" if planned else "plain", naux))
+        Jp, Kp = O.emul_df_jk(Bs.numpy(), nao, Cocc.numpy(), D.numpy(), O.slices_for_tol(tol))
+        J.copy_(torch.from_numpy(Jp))
+        K.copy_(torch.from_numpy(Kp))
+    return build
+
+
+def _worker_sharded(rank, world, port, out, naux, use_plan):
+    """df_jk_build_sharded itself on every rank: naux = 400 < 512 leaves rank 1 with an EMPTY shard
+    (it must contribute zeros and still take part in the all-reduce); plan= takes the planned call."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_2601_08077_b200 import binding
+    calls = []
+    binding.df_jk_build = _oracle_build(calls, False)
+    binding.df_jk_build_planned = _oracle_build(calls, True)
+    nao, nocc, tol = 20, 5, 1e-6
+    Bp = G.make_B_packed(nao, naux, seed=12)
+    Cocc = G.make_C_occ(nao, nocc, seed=12)
+    D = G.make_density(Cocc)
+    q0, q1 = sharded.shard_range(naux, rank, world)
+    Bs = torch.from_numpy(np.ascontiguousarray(Bp[:, q0:q1]))
+    J = torch.full((nao, nao), float("nan"), dtype=torch.float64)
+    K = torch.full((nao, nao), float("nan"), dtype=torch.float64)
+    sharded.df_jk_build_sharded(Bs, nao, q1 - q0, torch.from_numpy(Cocc), nocc, torch.from_numpy(D), tol, J, K,
+                                plan=object() if use_plan else None)
+    Jf, Kf = O.emul_df_jk(Bp, nao, Cocc, D, O.slices_for_tol(tol))
+    out.put((rank, q1 - q0, calls, O.rel_frobenius(J.numpy(), Jf), O.rel_frobenius(K.numpy(), Kf)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def _run_sharded(naux, use_plan):
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker_sharded, args=(r, 2, port, out, naux, use_plan)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted(out.get(timeout=240) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    return got
+
+
+def test_sharded_build_empty_shard_contributes_zeros():
+    (r0, n0, c0, eJ0, eK0), (r1, n1, c1, eJ1, eK1) = _run_sharded(400, False)
+    assert (n0, n1) == (400, 0)  # one 512-q block: rank 1 owns nothing
+    assert c0 == [("plain", 400)] and c1 == []  # no build call on the empty shard
+    # every rank ends with the full J, K (rank 1 contributed zeros, not NaN or stale data)
+    assert max(eJ0, eJ1) <= 1e-14 and max(eK0, eK1) <= 1e-14
+
+
+def test_sharded_build_plan_branch():
+    (r0, n0, c0, eJ0, eK0), (r1, n1, c1, eJ1, eK1) = _run_sharded(1300, True)
+    assert (n0, n1) == (1024, 276)
+    assert c0 == [("planned", 1024)] and c1 == [("planned", 276)]
+    assert max(eJ0, eJ1) <= 1e-14 and max(eK0, eK1) <= 1e-14
+
+
 def test_two_rank_allreduce_equals_single_build():
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
