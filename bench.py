@@ -1,17 +1,21 @@
 #!/usr/bin/env python
-"""bench.py -- DF J/K builds per second at nao = 1200 (BASELINE.json metric, config 3).
+"""bench.py -- DF J/K builds per second at nao = 1200 (BASELINE.json metric, configs[3]).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config large]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config large|medium|tiny|largest|gemm]
 
 A "step" is one pass of the whole hot path: one df_jk_build (rho, J, unpack+split, GEMM(5),
 X split, GEMM(6), K reduce) at that step's tolerance.  Step i takes entry i mod 12 of the
-synthetic 12-step SCF sequence D_k = D* + eps_k S_k of BASELINE.json config 2/3 (R11),
-whose tolerance tightens along Table 1 (paper_2601_08077_b200/policy.py), so the slice count
-adapts per step.  One JSON line on stdout; see DESIGN.md section 7 for every field.
+synthetic 12-step SCF sequence D_k = D* + eps_k S_k of BASELINE.json configs[2]/[3] (DESIGN.md
+R11), whose tolerance tightens along Table 1 (paper_2601_08077_b200/policy.py), so the slice count
+adapts per step.  `--config largest` (configs[4]) alternates its two tolerances 1e-6 / 1e-10 and
+reports the K build alone; `--config gemm` (configs[1]) is the standalone emulated-GEMM sweep.
+One JSON line on stdout; DESIGN.md section 7 explains every field.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import statistics
@@ -31,6 +35,8 @@ from df_inputs import generators as G  # noqa: E402
 NSEQ = 12
 METRIC = "df_jk_builds_per_s"
 UNIT = "builds/s"
+CONFIG_INDEX = {"tiny": 0, "gemm": 1, "medium": 2, "large": 3, "largest": 4}  # BASELINE.json configs[i]
+NCU_TABLE = os.path.join("profiles", "r02_ncu_kernels.csv")  # per-kernel ncu counters by slice count
 
 
 def flops_per_build(cfg):
@@ -48,6 +54,18 @@ def int8_ops_per_build(cfg, s):
     return pairs * g5, pairs * g6
 
 
+def unpack_bytes_per_build(cfg, s, with_j=True):
+    """Algorithmic HBM bytes of the unpack + split pass: packed B read once,
+    s digit planes of naux * nao rows of round_up(nao, 128) bytes written, and the chunk partials of
+    Eq. 4 (one double per packed pair and 32-q chunk) written by a plain build."""
+    npair = cfg.nao * (cfg.nao + 1) // 2
+    pitch = (cfg.nao + 127) // 128 * 128
+    b = 8.0 * npair * cfg.naux + float(s) * cfg.naux * cfg.nao * pitch
+    if with_j:
+        b += 8.0 * npair * ((cfg.naux + 31) // 32)
+    return b
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -55,6 +73,32 @@ def measured_peaks():
             d = json.load(f)
         return d, "measured"
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+
+
+def ncu_table():
+    """{(kernel class, s): row} from the committed ncu captures (profiles/r02_ncu_kernels.csv; the
+    commands that made it are in profiles/r02_ncu_summary.md).  Counters, not timings."""
+    path = os.path.join(ROOT, NCU_TABLE)
+    out = {}
+    if os.path.exists(path):
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                out[(row["kernel_class"], int(row["s"]))] = row
+    return out
+
+
+def traffic_for_mix(table, classes, used):
+    """Mean dram read+write bytes per launch of `classes` over the slice counts of the timed steps;
+    None when a slice count of the mix has no capture."""
+    tot, n = 0.0, 0
+    for s in used:
+        for c in classes:
+            row = table.get((c, s))
+            if row is None:
+                return None
+            tot += float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+            n += 1
+    return tot / n if n else None
 
 
 class ClockSampler:
@@ -108,9 +152,9 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def time_oracle_block(cfg, Bs, C, D, naux_sample):
-    """Seconds the oracle's plain FP64 J/K (oracle/df_oracle.py, as it stands) takes on
-    `naux_sample` auxiliary functions of the workload, on the host cores."""
+def oracle_plain_jk(cfg, Bs, C, D):
+    """The oracle's plain FP64 J/K (oracle/df_oracle.py, as it stands) on the auxiliary functions in
+    Bs, on the host cores.  Returns (seconds, J, K)."""
     from oracle import df_oracle as O
 
     t0 = time.perf_counter()
@@ -119,7 +163,7 @@ def time_oracle_block(cfg, Bs, C, D, naux_sample):
     K = O.df_k(Bs, cfg.nao, C)
     dt = time.perf_counter() - t0
     assert np.isfinite(J).all() and np.isfinite(K).all()
-    return dt
+    return dt, J, K
 
 
 def host_threads():
@@ -134,6 +178,14 @@ def host_threads():
     return len(os.sched_getaffinity(0))
 
 
+def workload_name(cfg_name, cfg=None):
+    idx = CONFIG_INDEX[cfg_name]
+    if cfg is None:
+        return f"gemm: emulated FP64 GEMM sweep, square M=N=K (BASELINE.json configs[{idx}])"
+    return (f"{cfg.name}: DF J/K build nao={cfg.nao} naux={cfg.naux} nocc={cfg.nocc} "
+            f"(BASELINE.json configs[{idx}])")
+
+
 def run_reference(args, cfg):
     """The reference arm for this tier = the CPU oracle, timed on the host cores; each step is
     a bounded sample (args.ref_q auxiliary functions) of the same workload, scaled to builds/s."""
@@ -144,18 +196,18 @@ def run_reference(args, cfg):
     C = G.make_C_occ(cfg.nao, cfg.nocc, cfg.seed)
     D = G.make_density(C)
     for _ in range(args.warmup):
-        time_oracle_block(cfg, Bs, C, D, qs)
-    dts = [time_oracle_block(cfg, Bs, C, D, qs) for _ in range(args.steps)]
+        oracle_plain_jk(cfg, Bs, C, D)
+    dts = [oracle_plain_jk(cfg, Bs, C, D)[0] for _ in range(args.steps)]
     t_build = (sum(dts) / len(dts)) * (cfg.naux / qs)
     value = 1.0 / t_build
     cores = host_threads()
-    sample = f"{qs} of {cfg.naux} auxiliary functions per step (plain FP64 rho, J, X, K), time scaled by naux/{qs}"
+    sample = (f"{qs} of {cfg.naux} auxiliary functions per step (plain FP64 rho, J, X, K), time EXTRAPOLATED "
+              f"by naux/{qs}")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_build, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{cfg.name}: DF J/K build nao={cfg.nao} naux={cfg.naux} nocc={cfg.nocc}",
-                   "sample": sample},
+        "config": {"workload": workload_name(args.config, cfg), "sample": sample},
         "effective_fp64_tflops": flops_per_build(cfg) * value / 1e12,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -186,9 +238,16 @@ def run_ours(args, cfg):
     B = G.make_B_packed_torch(nao, naux, cfg.seed + rank, device=dev)
     C0 = G.make_C_occ(nao, nocc, cfg.seed)
     D0 = G.make_density(C0)
-    seq = G.make_scf_sequence(D0, nocc, NSEQ, cfg.seed)
-    sched = policy.schedule([eps * eps for eps, _, _ in seq])[:NSEQ]  # dE_rel,k := eps_k^2 (R11)
-    tols = [t for _, t in sched]
+    if args.config == "largest":
+        # configs[4]: "Run with tol in {1e-6, 1e-10}": the two tolerances alternate, fixed C_occ / D
+        nseq = 2
+        seq = [(0.0, D0, C0), (0.0, D0, C0)]
+        tols = [1e-6, 1e-10]
+    else:
+        nseq = NSEQ
+        seq = G.make_scf_sequence(D0, nocc, NSEQ, cfg.seed)
+        sched = policy.schedule([eps * eps for eps, _, _ in seq])[:NSEQ]  # dE_rel,k := eps_k^2 (R11)
+        tols = [t for _, t in sched]
     slices = [p.df_slices_for_tol(t) for t in tols]
     D_dev = [torch.from_numpy(Dk).to(dev) for _, Dk, _ in seq]
     C_dev = [torch.from_numpy(Ck).to(dev) for _, _, Ck in seq]
@@ -210,7 +269,7 @@ def run_ours(args, cfg):
     plan_box = [None]  # set for the "planned" leg
 
     def step(i, resident):
-        k = i % NSEQ
+        k = i % nseq
         if resident:
             Dk, Ck = D_dev[k], C_dev[k]
         else:
@@ -239,6 +298,15 @@ def run_ours(args, cfg):
             dist.all_reduce(ms, op=dist.ReduceOp.MAX)
         return float(ms.item())
 
+    def profiled(nsteps, first):
+        """The same steps once more with the per-kernel-class CUDA-event brackets on (they add ~18
+        event pairs per build, so the headline leg runs without them)."""
+        p.df_profile_read()
+        p.df_profile_enable(True)
+        ms = timed(nsteps, True, first)
+        p.df_profile_enable(False)
+        return ms, p.df_profile_read()
+
     # own UTCIMMA issue-rate probe (MEASURED_PEAKS.json has no INT8 figure)
     probe_ms = p.df_debug_mma_peak(256, 20000, 148)
     int8_probe_tops = 2.0 * 128 * 256 * 32 * 20000 * 148 / probe_ms / 1e9
@@ -248,17 +316,19 @@ def run_ours(args, cfg):
     torch.cuda.synchronize()
     assert p.df_last_status() == 0, "status word set during warm-up"
 
+    # ---- headline: K timed steps, inputs resident, no profiling brackets
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
     n0 = p.df_launch_count()
-    p.df_profile_enable(True)
     ms_total = timed(args.steps, True, args.warmup)
-    p.df_profile_enable(False)
     launches = p.df_launch_count() - n0
-    prof = p.df_profile_read()
     clocks = sampler.stop() if rank == 0 else None
     assert p.df_last_status() == 0 and bool(torch.isfinite(K).all()) and bool(torch.isfinite(J).all())
+    assert bool(torch.equal(K, K.T)) and bool(torch.equal(J, J.T))
+
+    # ---- the same steps with per-kernel-class timing (roofline numerators)
+    ms_prof, prof = profiled(args.steps, args.warmup)
 
     # ---- end to end through the C-ABI with HOST buffers: D_k, C_k from pinned memory in, J, K
     # out, every step; B stays resident (it is constant over the SCF).
@@ -266,6 +336,7 @@ def run_ours(args, cfg):
     ms_e2e = timed(args.steps, False, args.warmup)
     h2d = (nao * nao + nao * nocc) * 8
     d2h = 2 * nao * nao * 8
+    last = (args.warmup + args.steps - 1) % nseq  # the step J, K now hold
 
     # ---- planned leg: B split once into max(slices) planes outside the
     # timed region, the same steps with GEMM(5) reading the plan.  An extra, not the headline:
@@ -290,10 +361,8 @@ def run_ours(args, cfg):
         torch.cuda.synchronize()
         for i in range(args.warmup):
             step(i, True)
-        p.df_profile_enable(True)
         ms_planned = timed(args.steps, True, args.warmup)
-        p.df_profile_enable(False)
-        prof_planned = p.df_profile_read()
+        _, prof_planned = profiled(args.steps, args.warmup)
         ms_planned_e2e = timed(args.steps, False, args.warmup)
         same = bool(torch.equal(J, J_ref)) and bool(torch.equal(K, K_ref))
         assert p.df_last_status() == 0
@@ -316,24 +385,32 @@ def run_ours(args, cfg):
     units = args.steps * world  # shard-builds of this config processed by all ranks
     value = units / (ms_total / 1e3)
     e2e_value = units / (ms_e2e / 1e3)
-    used = [slices[i % NSEQ] for i in range(args.warmup, args.warmup + args.steps)]
+    used = [slices[i % nseq] for i in range(args.warmup, args.warmup + args.steps)]
     ops5 = sum(int8_ops_per_build(cfg, s)[0] for s in used)
     ops6 = sum(int8_ops_per_build(cfg, s)[1] for s in used)
     ms5, n5 = prof["gemm5_i8"]
     ms6, n6 = prof["gemm6_i8"]
+    msu, nu = prof["jk_unpack_split"]
     peaks, peak_kind = measured_peaks()
+    table = ncu_table()
     # INT8 dense peak = measured bf16 peak x the nominal INT8:bf16 ratio (4.5 : 2.25 PFLOP/s);
     # the GEMMs run inside a long step, so the sustained figure applies.
     peak_tops = 2.0 * peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
     achieved = (ops5 + ops6) / ((ms5 + ms6) / 1e3) / 1e12
+    ubytes = sum(unpack_bytes_per_build(cfg, s) for s in used)
+    hbm_achieved = ubytes / (msu / 1e3) / 1e9 if msu else None
+
+    def pipe_pct(cls):
+        v = {str(s): float(table[(cls, s)]["tensor_pipe_active_pct"]) for s in sorted(set(used)) if (cls, s) in table}
+        return v or None
+
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "int8", "dtype_note": "int8 x int8 -> int32 slice-pair products, f64 recombination; J in f64",
         "data": "synthetic",
-        "config": {"workload": f"{cfg.name}: DF J/K build nao={nao} naux={naux} nocc={nocc} (BASELINE.json configs[3]), "
-                               f"12-step adaptive SCF sequence, one q-shard per GPU",
-                   "slices_per_step": used, "tol_per_step": [tols[i % NSEQ] for i in range(args.warmup, args.warmup + args.steps)],
+        "config": {"workload": workload_name(args.config, cfg) + (", 12-step adaptive SCF sequence" if nseq == NSEQ else ", tol alternating 1e-6 / 1e-10") + ", one q-shard per GPU",
+                   "slices_per_step": used, "tol_per_step": [tols[i % nseq] for i in range(args.warmup, args.warmup + args.steps)],
                    "l2": "inputs larger than L2: packed B is %.1f GB and every step streams it" % (B.numel() * 8 / 1e9),
                    "workspace_gb": ws.view.numel() / 1e9, "q_blocks_per_launch": nblk},
         "effective_fp64_tflops": flops_per_build(cfg) * value / 1e12,
@@ -348,28 +425,198 @@ def run_ours(args, cfg):
                      "achieved_gemm6": ops6 / (ms6 / 1e3) / 1e12 if ms6 else None,
                      "int8_probe_tops": int8_probe_tops, "frac_of_probe": achieved / int8_probe_tops,
                      "launches": n5 + n6, "avg_launch_ms": (ms5 + ms6) / max(1, n5 + n6),
-                     "share_of_step": (ms5 + ms6) / ms_total,
-                     # dram__bytes_read+write per launch, ncu --set full at s = 4 (profiles/r01_ncu_summary.md):
-                     # GEMM(5) 25.9 + 6.1 GB, GEMM(6) 4.5 + 0.2 GB -> mean over the two launches of a build
-                     "traffic": 0.5 * (32.0e9 + 4.7e9), "traffic_unit": "bytes per launch (s = 4)"},
+                     "share_of_step": (ms5 + ms6) / ms_prof,
+                     "traffic": traffic_for_mix(table, ("gemm5_i8", "gemm6_i8"), used),
+                     "traffic_unit": "dram read + write bytes per launch, mean over the two GEMM launches of the timed "
+                                     "steps' slice counts",
+                     "traffic_source": NCU_TABLE if table else None,
+                     "ncu_tensor_pipe_active_pct_gemm5": pipe_pct("gemm5_i8"),
+                     "ncu_tensor_pipe_active_pct_gemm6": pipe_pct("gemm6_i8")},
+        "roofline_hbm": {"bound": "hbm", "kernel": "jk_unpack_split_kernel (+ the chunk partials of Eq. 4)",
+                         "achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                         "frac": hbm_achieved / peaks["hbm_gbs"] if hbm_achieved else None,
+                         "peak_source": f"hbm_gbs of MEASURED_PEAKS.json ({peak_kind}; copy bandwidth)",
+                         "launches": nu, "avg_launch_ms": msu / max(1, nu), "share_of_step": msu / ms_prof,
+                         "traffic": traffic_for_mix(table, ("jk_unpack_split",), used),
+                         "traffic_source": NCU_TABLE if table else None},
         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items() if v[1]},
+        "profiled_ms_per_step": ms_prof / args.steps,
     }
+    if args.config == "largest":
+        # configs[4]: "a single K build reported separately": everything but rho and J (pass A, the
+        # J reduction) of one build, per tolerance, from the per-class brackets of the profiled pass
+        kcls = ("split", "jk_unpack_split", "gemm5_i8", "jk_split_x", "gemm6_i8", "jk_k_reduce")
+        kb = {}
+        for k in range(nseq):
+            p.df_profile_read()
+            p.df_profile_enable(True)
+            for _ in range(2):
+                step(k, True)
+            torch.cuda.synchronize()
+            p.df_profile_enable(False)
+            pr = p.df_profile_read()
+            kms = sum(pr[c][0] for c in kcls) / 2
+            kflops = 4.0 * nao**2 * naux * nocc
+            kb[f"tol={tols[k]:g}"] = {"slices": slices[k], "k_build_ms": kms,
+                                      "k_effective_fp64_tflops": kflops / (kms / 1e3) / 1e12,
+                                      "kernel_ms": {c: pr[c][0] / 2 for c in kcls},
+                                      "note": "the unpack + split pass also carries the chunk partials of J (Eq. 4)"}
+        out["k_build"] = kb
     if planned is not None:
         planned["effective_fp64_tflops"] = flops_per_build(cfg) * planned["value"] / 1e12
         out["planned"] = planned
     if world == 1 and not args.no_cpu_baseline:
+        # ---- CPU baseline = the oracle as it stands on a bounded q-sample of the same B, and the
+        # parity check of this run: the CUDA path builds J, K over the SAME sample (same bytes, the
+        # C_occ / D and tolerance of the last timed step) and must match the oracle's full matrices.
         qs = min(args.cpu_q, naux)
-        Bs = B[:, :qs].contiguous().cpu().numpy()
-        dt = time_oracle_block(cfg, Bs, C0, D0, qs)
+        Bs_dev = B[:, :qs].contiguous()
+        Ck, Dk = seq[last][2], seq[last][1]
+        dt, J_o, K_o = oracle_plain_jk(cfg, Bs_dev.cpu().numpy(), Ck, Dk)
         v = 1.0 / (dt * naux / qs)
+        Jg, Kg = torch.empty_like(J), torch.empty_like(K)
+        p.df_jk_build(Bs_dev, nao, qs, C_dev[last], nocc, D_dev[last], tols[last], Jg, Kg)
+        torch.cuda.synchronize()
+        eJ = float(np.linalg.norm(Jg.cpu().numpy() - J_o) / np.linalg.norm(J_o))
+        eK = float(np.linalg.norm(Kg.cpu().numpy() - K_o) / np.linalg.norm(K_o))
+        assert eJ <= 1e-12 and eK <= tols[last], (eJ, eK, tols[last])
+        del Bs_dev
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
                                "sample": f"first {qs} of {naux} auxiliary functions of the same B (plain FP64 "
-                                         f"rho, J, X, K; {dt:.1f} s), time scaled by naux/{qs}",
+                                         f"rho, J, X, K; {dt:.1f} s), time EXTRAPOLATED by naux/{qs}",
                                "effective_fp64_tflops": flops_per_build(cfg) * v / 1e12}
+        out["parity_check"] = {"what": f"df_jk_build over the same {qs} auxiliary functions against the oracle's plain "
+                                       f"FP64 J, K (full matrices, rel. Frobenius)", "tol": tols[last],
+                               "slices": slices[last], "J_relF": eJ, "K_relF": eK, "passed": True}
+    if world == 1 and args.level0 and args.config in ("large", "medium", "tiny"):
+        # ---- level 0 of Table 1 ("standard FP64") runs as the s = 8 emulation
+        # (policy.py); reported separately: it is not part of the 12-step sequence
+        ws.close()
+        del ws
+        torch.cuda.empty_cache()
+        tol0 = 2.0 ** -52
+        s0 = p.df_slices_for_tol(tol0)
+        nb0 = (naux + 511) // 512
+        free, _ = torch.cuda.mem_get_info(dev)
+        while nb0 > 1 and p.df_jk_workspace_bytes_blocks(nao, naux, nocc, s0, nb0) > free - (4 << 30):
+            nb0 -= 1
+        ws0 = p.Workspace(p.df_jk_workspace_bytes_blocks(nao, naux, nocc, s0, nb0), device=dev)
+        for _ in range(2):
+            p.df_jk_build(B, nao, naux, C_dev[last], nocc, D_dev[last], tol0, J, K)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(3):
+            p.df_jk_build(B, nao, naux, C_dev[last], nocc, D_dev[last], tol0, J, K)
+        e1.record()
+        torch.cuda.synchronize()
+        ms0 = e0.elapsed_time(e1) / 3
+        out["level0"] = {"tol": tol0, "slices": s0, "ms_per_build": ms0,
+                         "effective_fp64_tflops": flops_per_build(cfg) / (ms0 / 1e3) / 1e12,
+                         "note": "Table 1 level 0 as the s = 8 emulation (at least FP64-accurate, "
+                                 "tests/test_oracle_emulation.py); B200 native FP64 peak is ~37-40 TFLOP/s"}
+        ws0.close()
+    else:
+        ws.close()
     print(json.dumps(out))
-    ws.close()
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_gemm(args):
+    """BASELINE.json configs[1]: C = A.B emulated with s = 1..8 slices, square M = N = K.  Per (N, s):
+    whole-call ms, the split kernels and the INT8 GEMM launch separately (CUDA-event brackets, warm-up
+    excluded), INT8 TOP/s against 2 x the measured bf16 BURST peak (each GEMM is timed alone), rel.
+    Frobenius error against torch's FP64 matmul on the same device, and that native FP64 (cuBLAS
+    DGEMM) time as context only -- it is not on the hot path."""
+    import torch
+
+    import paper_2601_08077_b200 as p
+
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    sizes = args.sizes
+    slices = list(range(1, 9))
+    nmax = max(sizes)
+    ws = p.Workspace(p.df_emul_gemm_workspace_bytes(nmax, nmax, nmax, 8), device=dev)
+    peaks, peak_kind = measured_peaks()
+    peak_tops = 2.0 * peaks["bf16_tflops"]
+    reps = max(1, args.steps)
+
+    def timed(fn):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    sampler = ClockSampler(0)
+    sampler.start()
+    n0 = p.df_launch_count()
+    sweep = []
+    for n in sizes:
+        if n <= 4096:
+            A, B = (torch.from_numpy(x).to(dev) for x in G.make_gemm_inputs(n, n, n, seed=n))
+        else:  # same distribution (DESIGN.md R10), generated on the device
+            g = torch.Generator(device=dev)
+            g.manual_seed(n)
+
+            def one():
+                e = torch.rand((n, n), generator=g, dtype=torch.float64, device=dev) * 30.0 - 30.0
+                off = torch.randint(-10, 11, (n, 1), generator=g, device=dev).to(torch.float64)
+                sgn = torch.where(torch.rand((n, n), generator=g, device=dev) < 0.5, -1.0, 1.0).to(torch.float64)
+                return sgn * torch.exp2(e + off)
+
+            A, B = one(), one()
+        C = torch.empty((n, n), dtype=torch.float64, device=dev)
+        ref = A @ B
+        torch.matmul(A, B, out=ref)
+        t_native = timed(lambda: torch.matmul(A, B, out=ref))
+        ref_norm = float(torch.linalg.norm(ref))
+        for s in slices:
+            for _ in range(max(1, args.warmup)):  # warm-up calls, outside every average
+                p.df_emul_gemm_slices(A, B, C, n, n, n, s)
+            torch.cuda.synchronize()
+            t_all = timed(lambda: p.df_emul_gemm_slices(A, B, C, n, n, n, s))
+            p.df_profile_read()
+            p.df_profile_enable(True)
+            timed(lambda: p.df_emul_gemm_slices(A, B, C, n, n, n, s))
+            p.df_profile_enable(False)
+            prof = p.df_profile_read()
+            t_gemm = prof["emul_gemm_i8"][0] / max(1, prof["emul_gemm_i8"][1])
+            t_split = prof["split"][0] / max(1, prof["split"][1])
+            err = float(torch.linalg.norm(C - ref)) / ref_norm
+            ops = 2.0 * n**3 * s * (s + 1) / 2
+            tops = ops / t_gemm / 1e9
+            sweep.append({"N": n, "s": s, "ms": t_all, "split_ms": t_split, "gemm_ms": t_gemm,
+                          "int8_tops": tops, "frac": tops / peak_tops,
+                          "effective_fp64_tflops": 2.0 * n**3 / t_all / 1e9, "relF_vs_native_fp64": err,
+                          "native_fp64_ms": t_native,
+                          "split_gbs": (2.0 * n * n * (8 + s)) / t_split / 1e6})
+        del A, B, C, ref
+    launches = p.df_launch_count() - n0
+    clocks = sampler.stop()
+    head = [r for r in sweep if r["N"] == nmax and r["s"] == 4][0]
+    print(json.dumps({
+        "metric": "df_emul_gemm_effective_fp64_tflops", "value": head["effective_fp64_tflops"], "unit": "TFLOP/s",
+        "n_gpus": 1, "steps": reps, "warmup": max(1, args.warmup), "ms_per_step": head["ms"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8",
+        "dtype_note": "int8 x int8 -> int32 slice-pair products, f64 recombination", "data": "synthetic",
+        "config": {"workload": workload_name("gemm") + f", headline N={nmax} s=4; sizes {sizes}, s = 1..8",
+                   "l2": "operand planes of the headline size are %.1f GB, larger than L2" % (2 * 4 * nmax * nmax / 1e9)},
+        "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": {"bound": "tensor", "kernel": f"gemm_i8_kernel (df_emul_gemm, N={nmax}, s=4)",
+                     "achieved": head["int8_tops"], "peak": peak_tops, "unit": "TOP/s", "frac": head["frac"],
+                     "peak_source": f"2 x bf16_tflops (burst) of MEASURED_PEAKS.json ({peak_kind}): timed alone",
+                     "traffic": None},
+        "sweep": sweep,
+    }))
+    ws.close()
 
 
 def main():
@@ -378,12 +625,20 @@ def main():
     ap.add_argument("--steps", type=int, default=12)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="large", choices=sorted(G.CONFIGS))
-    ap.add_argument("--ref-q", dest="ref_q", type=int, default=32)
-    ap.add_argument("--cpu-q", dest="cpu_q", type=int, default=256)
+    ap.add_argument("--config", default="large", choices=sorted(CONFIG_INDEX))
+    ap.add_argument("--ref-q", dest="ref_q", type=int, default=128)
+    ap.add_argument("--cpu-q", dest="cpu_q", type=int, default=512)
+    ap.add_argument("--sizes", type=int, nargs="+", default=[1024, 2048, 4096, 8192, 16384])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-level0", dest="level0", action="store_false")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.config == "gemm":
+        if args.impl == "reference":
+            print(json.dumps({"impl": "reference", "unavailable": "the reference arm is defined for the DF J/K configs"}))
+            return
+        run_gemm(args)
+        return
     cfg = G.CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, cfg)
