@@ -140,7 +140,8 @@ static GemmWs carve_gemm(void* base, int64_t m, int64_t n, int64_t k, int s) {
 static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, int s,
                           cudaStream_t st) {
   if (!A || !B || !C) return DF_ERR_NULL;
-  if (m <= 0 || n <= 0 || k <= 0 || k > (1ll << 30) || m > (1ll << 31) || n > (1ll << 31)) return DF_ERR_DIM;
+  // n: the column split puts 32-column blocks on grid.y (65535)
+  if (m <= 0 || n <= 0 || k <= 0 || k > (1ll << 30) || m >= (1ll << 31) || n > 65535ll * 32) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
   if (!device_ok()) return DF_ERR_DEVICE;
   if (!g_ws) return DF_ERR_WORKSPACE;
@@ -638,7 +639,7 @@ int df_debug_split_rows(const double* X, int64_t rows, int64_t cols, int s, int3
 
 int df_debug_split_cols(const double* X, int64_t k, int64_t n, int s, int32_t* e, int8_t* planes, void* stream) {
   if (!X || !e || !planes) return DF_ERR_NULL;
-  if (k <= 0 || n <= 0) return DF_ERR_DIM;
+  if (k <= 0 || n <= 0 || k > (1ll << 30) || n > 65535ll * 32) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
   if (!device_ok()) return DF_ERR_DEVICE;
   if (!g_ws || g_ws_bytes < 256 + round_up(4 * n, 256)) return DF_ERR_WORKSPACE;

@@ -1,6 +1,11 @@
 // split.cu -- FP64 -> scale index + balanced INT8 digit planes (rows H1, H2 of SURVEY.md 8(a)).
-// HBM-bound passes: 8 B read + s B written per element (rows), the row re-read for the digit
-// pass hits L2 because the same block has just streamed it for the maximum.
+// HBM-bound passes: 8 B read + s B written per element.  Rows: a block streams its row twice (the
+// maximum, then the digits; the second read hits L2) with 256-bit loads, stages the digit bytes in
+// shared memory and writes whole 1 KB runs per plane.  Columns (the transposing split): column
+// maxima in one pass over the matrix, then 128-row x 32-column tiles: lane = column (256-byte runs
+// per load instruction), 16 bytes per plane and thread into a staging tile, whole 128-byte lines of
+// planes[t][column][k ..] out.  The scalar kernels below them serve operands whose rows are not
+// 32-byte aligned.
 //
 // Definition (R2; PAPER.md:130 is silent on the internals):
 //   e   = scale index of max_k |x| (common.cuh: scale_index_from_hi)
@@ -78,12 +83,12 @@ __global__ void __launch_bounds__(256) split_rows_kernel(const double* __restric
   }
 }
 
-// Column maxima of a k x n row-major matrix: thread per column, grid.y over row chunks.
+// Column maxima of a k x n row-major matrix: thread per column, grid.x over row chunks (odd n).
 __global__ void __launch_bounds__(256) col_max_kernel(const double* __restrict__ X, long long k, long long n,
                                                       int rows_per_block, uint32_t* __restrict__ cmax) {
-  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long c = (long long)blockIdx.y * blockDim.x + threadIdx.x;
   if (c >= n) return;
-  const long long r0 = (long long)blockIdx.y * rows_per_block;
+  const long long r0 = (long long)blockIdx.x * rows_per_block;
   const long long r1 = min(k, r0 + rows_per_block);
   uint32_t hm = 0;
   for (long long r = r0; r < r1; ++r) hm = max(hm, abs_hi_word(__ldg(X + r * n + c)));
@@ -100,36 +105,158 @@ __global__ void col_scale_kernel(const uint32_t* __restrict__ cmax, long long n,
   if (stt) atomicOr(status, stt);
 }
 
-// Transposing split of a k x n matrix: lane <-> column (coalesced 256 B reads along n), each
-// thread converts 32 consecutive k of its column and writes 32 B per plane to
-// planes[t][col][k0 .. k0+31].  Block = 32 columns x 8 k-runs.
+// ---------------------------------------------------------------------------
+// Vectorised row split: ld % 4 == 0 and a 32-byte aligned base.  One block per row.
+// ---------------------------------------------------------------------------
+constexpr int kRowChunk = 1024;  // elements per block iteration: 256 threads x 4
 template <int S>
-__global__ void __launch_bounds__(256) split_cols_kernel(const double* __restrict__ X, long long k, long long n,
-                                                         const int32_t* __restrict__ e,
-                                                         int8_t* __restrict__ planes, long long pitch,
-                                                         long long plane_stride) {
-  const long long c = (long long)blockIdx.x * 32 + (threadIdx.x & 31);
-  const long long k0 = ((long long)blockIdx.y * 8 + (threadIdx.x >> 5)) * 32;
-  if (c >= n || k0 >= pitch) return;
-  const double scale = pow2_double(63 - e[c]);
-  uint32_t w[S][8];
+__global__ void __launch_bounds__(256) split_rows_v4_kernel(const double* __restrict__ X, long long cols, long long ld,
+                                                            int32_t* __restrict__ e, int8_t* __restrict__ planes,
+                                                            long long pitch, long long plane_stride,
+                                                            int* __restrict__ status) {
+  const long long row = blockIdx.x;
+  const double* x = X + row * ld;
+  __shared__ uint32_t wmax[8];
+  __shared__ int e_sh;
+  __shared__ __align__(16) uint32_t stage[2][S][256];  // [buffer][plane][thread]: 4 digit bytes per thread
+  const int tid = threadIdx.x;
+  const long long nvec = cols >> 2;  // whole 4-element vectors
+  uint32_t hm = 0;
+  {
+    long long v = tid;
+    for (; v + 768 < nvec; v += 1024) {  // four 256-bit loads in flight per thread
+      double a[16];
 #pragma unroll
-  for (int t = 0; t < S; ++t)
+      for (int u = 0; u < 4; ++u) ldg_nc_v4f64(x + 4 * (v + 256 * u), a[4 * u], a[4 * u + 1], a[4 * u + 2], a[4 * u + 3]);
 #pragma unroll
-    for (int j = 0; j < 8; ++j) w[t][j] = 0;
-#pragma unroll
-  for (int j = 0; j < 32; ++j) {
-    const long long r = k0 + j;
-    const double v = (r < k) ? __ldg(X + r * n + c) : 0.0;
-    const uint64_t dg = balanced_digits(v, scale);
-#pragma unroll
-    for (int t = 0; t < S; ++t) w[t][j >> 2] = put_byte(w[t][j >> 2], digit_byte(dg, t), j & 3);
+      for (int j = 0; j < 16; ++j) hm = max(hm, abs_hi_word(a[j]));
+    }
+    for (; v < nvec; v += 256) {
+      double a0, a1, a2, a3;
+      ldg_nc_v4f64(x + 4 * v, a0, a1, a2, a3);
+      hm = max(max(hm, abs_hi_word(a0)), max(abs_hi_word(a1), max(abs_hi_word(a2), abs_hi_word(a3))));
+    }
+    for (long long c = 4 * nvec + tid; c < cols; c += 256) hm = max(hm, abs_hi_word(__ldg(x + c)));
   }
+  hm = warp_max_u32(hm);
+  if ((tid & 31) == 0) wmax[tid >> 5] = hm;
+  __syncthreads();
+  if (tid == 0) {
+    uint32_t m = 0;
+    for (int i = 0; i < 8; ++i) m = max(m, wmax[i]);
+    const int ee = scale_index_from_hi(m);
+    e_sh = ee;
+    e[row] = ee;
+    const int stt = status_from_hi(m);
+    if (stt) atomicOr(status, stt);
+  }
+  __syncthreads();
+  const double scale = pow2_double(63 - e_sh);
+  int8_t* const prow = planes + row * pitch;
+  int buf = 0;
+  for (long long c0 = 0; c0 < pitch; c0 += kRowChunk, buf ^= 1) {
+    const long long c = c0 + 4 * tid;
+    double a[4] = {0.0, 0.0, 0.0, 0.0};
+    if (c + 3 < cols) {
+      ldg_nc_v4f64(x + c, a[0], a[1], a[2], a[3]);
+    } else {
 #pragma unroll
-  for (int t = 0; t < S; ++t) {
-    uint4* dst = reinterpret_cast<uint4*>(planes + t * plane_stride + c * pitch + k0);
-    dst[0] = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
-    dst[1] = make_uint4(w[t][4], w[t][5], w[t][6], w[t][7]);
+      for (int j = 0; j < 4; ++j)
+        if (c + j < cols) a[j] = __ldg(x + c + j);
+    }
+    uint32_t hi[4], lo[4], ph[4], pl[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const uint64_t dg = balanced_digits(a[j], scale);
+      hi[j] = (uint32_t)(dg >> 32);
+      lo[j] = (uint32_t)dg;
+    }
+    transpose4x4_bytes(hi, ph);
+    if (S > 4) transpose4x4_bytes(lo, pl);
+#pragma unroll
+    for (int t = 0; t < S; ++t) stage[buf][t][tid] = (t < 4) ? ph[3 - t] : pl[7 - t];
+    __syncthreads();  // one barrier per chunk: buffer buf ^ 1 was last read before this barrier
+    // S planes x 1 KB: 64 sixteen-byte vectors per plane, whole runs per plane
+    for (int idx = tid; idx < S * 64; idx += 256) {
+      const int t = idx >> 6, v = idx & 63;
+      const long long col = c0 + 16 * v;
+      if (col < pitch)
+        *reinterpret_cast<uint4*>(prow + t * plane_stride + col) = *reinterpret_cast<const uint4*>(&stage[buf][t][4 * v]);
+    }
+  }
+}
+
+// Column maxima, two columns per thread (16-byte loads), rows in chunks over grid.x.
+__global__ void __launch_bounds__(256) col_max_v2_kernel(const double* __restrict__ X, long long k, long long n,
+                                                         int rows_per_block, uint32_t* __restrict__ cmax) {
+  const long long c = ((long long)blockIdx.y * blockDim.x + threadIdx.x) * 2;
+  if (c >= n) return;
+  const long long r0 = (long long)blockIdx.x * rows_per_block;
+  const long long r1 = min(k, r0 + rows_per_block);
+  uint32_t h0 = 0, h1 = 0;
+  long long r = r0;
+  for (; r + 8 <= r1; r += 8) {  // eight loads in flight
+    double2 v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = __ldg(reinterpret_cast<const double2*>(X + (r + u) * n + c));
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      h0 = max(h0, abs_hi_word(v[u].x));
+      h1 = max(h1, abs_hi_word(v[u].y));
+    }
+  }
+  for (; r < r1; ++r) {
+    const double2 v = __ldg(reinterpret_cast<const double2*>(X + r * n + c));
+    h0 = max(h0, abs_hi_word(v.x));
+    h1 = max(h1, abs_hi_word(v.y));
+  }
+  atomicMax(&cmax[c], h0);
+  atomicMax(&cmax[c + 1], h1);
+}
+
+// Transposing split in 128-row x 32-column tiles: lane = column, warp = 16-row group.  A thread loads
+// its 16 values (a warp instruction reads one 256-byte run of a row), converts them with its column's
+// scale and writes 16 bytes per plane into the staging tile [plane][column][128 + 16]; after the
+// barrier 8 lanes copy each 128-byte line planes[t][column][k0 .. k0 + 127] out.
+constexpr int kColPitch = 144;
+template <int S>
+__global__ void __launch_bounds__(256) split_cols_tile_kernel(const double* __restrict__ X, long long k, long long n,
+                                                              const int32_t* __restrict__ e,
+                                                              int8_t* __restrict__ planes, long long pitch,
+                                                              long long plane_stride) {
+  __shared__ __align__(16) uint8_t tile[S * 32 * kColPitch];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long c0 = (long long)blockIdx.y * 32;
+  const long long k0 = (long long)blockIdx.x * 128;
+  const long long c = c0 + lane;
+  const bool c_ok = c < n;
+  const double scale = pow2_double(63 - (c_ok ? e[c] : 0));
+  const long long r0 = k0 + warp * 16;
+  double x[16];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) x[j] = (c_ok && r0 + j < k) ? __ldg(X + (r0 + j) * n + c) : 0.0;
+#pragma unroll
+  for (int g4 = 0; g4 < 4; ++g4) {
+    uint32_t hi[4], lo[4], ph[4], pl[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const uint64_t dg = balanced_digits(x[4 * g4 + j], scale);
+      hi[j] = (uint32_t)(dg >> 32);
+      lo[j] = (uint32_t)dg;
+    }
+    transpose4x4_bytes(hi, ph);
+    if (S > 4) transpose4x4_bytes(lo, pl);
+#pragma unroll
+    for (int t = 0; t < S; ++t)
+      *reinterpret_cast<uint32_t*>(tile + (t * 32 + lane) * kColPitch + warp * 16 + g4 * 4) = (t < 4) ? ph[3 - t] : pl[7 - t];
+  }
+  __syncthreads();
+  for (int idx = warp * 4 + (lane >> 3); idx < S * 32; idx += 32) {
+    const int t = idx >> 5, cc = idx & 31;
+    const long long kk = k0 + (lane & 7) * 16;
+    if (c0 + cc < n && kk < pitch)
+      *reinterpret_cast<uint4*>(planes + t * plane_stride + (c0 + cc) * pitch + kk) =
+          *reinterpret_cast<const uint4*>(tile + (t * 32 + cc) * kColPitch + (lane & 7) * 16);
   }
 }
 
@@ -149,6 +276,13 @@ cudaError_t launch_split_rows(const double* X, int64_t rows, int64_t cols, int64
                               int8_t* planes, int64_t pitch, int64_t plane_stride, int* status,
                               cudaStream_t st) {
   if (rows <= 0) return cudaSuccess;
+  if (ld % 4 == 0 && ((uintptr_t)X & 31) == 0 && pitch % 16 == 0 && plane_stride % 16 == 0 &&
+      ((uintptr_t)planes & 15) == 0) {
+    DFE_DISPATCH_S(s, (split_rows_v4_kernel<SS><<<(unsigned)rows, 256, 0, st>>>(X, cols, ld, e, planes, pitch,
+                                                                              plane_stride, status)));
+    count_launch();
+    return cudaGetLastError();
+  }
   DFE_DISPATCH_S(s, (split_rows_kernel<SS><<<(unsigned)rows, 256, 0, st>>>(X, rows, cols, ld, e, planes, pitch,
                                                                          plane_stride, status)));
   count_launch();
@@ -160,12 +294,22 @@ cudaError_t launch_split_cols(const double* X, int64_t k, int64_t n, int s, uint
                               cudaStream_t st) {
   cudaError_t err = cudaMemsetAsync(cmax, 0, sizeof(uint32_t) * n, st);
   if (err != cudaSuccess) return err;
-  const int rows_per_block = 64;
-  dim3 g1((unsigned)((n + 255) / 256), (unsigned)((k + rows_per_block - 1) / rows_per_block));
-  col_max_kernel<<<g1, 256, 0, st>>>(X, k, n, rows_per_block, cmax);
+  // row chunks ride on grid.x (2^31 - 1 blocks), column blocks on grid.y: k up to the 2^30 the entry points
+  // accept and n up to 2^31 stay inside the grid limits
+  const int rows_per_block = 128;
+  const unsigned kchunks = (unsigned)((k + rows_per_block - 1) / rows_per_block);
+  if ((n + 31) / 32 > 65535) return cudaErrorInvalidValue;
+  if (n % 2 == 0 && ((uintptr_t)X & 15) == 0) {
+    dim3 g1(kchunks, (unsigned)((n / 2 + 255) / 256));
+    col_max_v2_kernel<<<g1, 256, 0, st>>>(X, k, n, rows_per_block, cmax);
+  } else {
+    dim3 g1(kchunks, (unsigned)((n + 255) / 256));
+    col_max_kernel<<<g1, 256, 0, st>>>(X, k, n, rows_per_block, cmax);
+  }
   col_scale_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cmax, n, e, status);
-  dim3 g2((unsigned)((n + 31) / 32), (unsigned)((pitch / 32 + 7) / 8));
-  DFE_DISPATCH_S(s, (split_cols_kernel<SS><<<g2, 256, 0, st>>>(X, k, n, e, planes, pitch, plane_stride)));
+  if (pitch % 16 != 0 || plane_stride % 16 != 0 || ((uintptr_t)planes & 15) != 0) return cudaErrorInvalidValue;
+  dim3 g2((unsigned)((pitch + 127) / 128), (unsigned)((n + 31) / 32));
+  DFE_DISPATCH_S(s, (split_cols_tile_kernel<SS><<<g2, 256, 0, st>>>(X, k, n, e, planes, pitch, plane_stride)));
   count_launch(3);
   return cudaGetLastError();
 }
