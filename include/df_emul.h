@@ -21,8 +21,12 @@
  *  - `stream` is a cudaStream_t passed as void* (NULL = the default stream).
  *    Work is enqueued on it; no entry point synchronises with the host unless it
  *    says so.  Results are valid once the stream has reached the end of the call.
- *  - Scratch memory comes from ONE caller-supplied workspace registered with
- *    df_set_workspace(); one workspace serves one stream at a time.
+ *  - Scratch memory comes from a caller-supplied workspace.  A CONTEXT (df_context_create) binds one
+ *    workspace on one device together with its policy mode, debug knobs and cached tensor maps; one
+ *    context serves one stream at a time, and several contexts (each with its own workspace) may run
+ *    concurrently on several streams.  The entry points without a context argument use a process-wide
+ *    default context whose workspace is registered with df_set_workspace().  A call made while another
+ *    device is current than the one the workspace was registered on returns DF_ERR_DEVICE.
  *  - Return value: DF_OK (0) or a negative DF_ERR_* code.  No exceptions, no
  *    printing.  Data-dependent faults (Inf/NaN, out-of-range magnitudes) do not
  *    fail the call: they set bits in a device status word, see df_last_status().
@@ -67,7 +71,7 @@ int df_num_int8_gemms(int s);
  * 32*floor(131071/(32 s))  (R4). */
 int df_kflush(int s);
 
-/* Select the tol -> s mapping used by df_emul_gemm / df_jk_build. */
+/* Select the tol -> s mapping used by df_emul_gemm / df_jk_build (default context). */
 int df_set_policy_mode(int mode);
 
 /* ---- workspace ---------------------------------------------------------- */
@@ -84,11 +88,45 @@ int64_t df_jk_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, int s);
  * = the whole auxiliary range in one super-block). */
 int64_t df_jk_workspace_bytes_blocks(int64_t nao, int64_t naux, int64_t nocc, int s, int64_t nblocks);
 
-/* Register a device buffer (256-byte aligned) as THE workspace.  The library
- * never frees it.  Passing NULL/0 unregisters it. */
+/* Register a device buffer (256-byte aligned, on the current device) as the workspace of the
+ * default context.  The library never frees it.  Passing NULL/0 unregisters it. */
 int df_set_workspace(void* ptr, int64_t bytes);
 
-/* ---- the two mandated entry points -------------------------------------- */
+/* ---- contexts: one workspace per concurrent stream ---------- */
+
+typedef struct df_context df_context;
+
+/* Creates a context on the CURRENT device with `workspace` (device memory, 256-byte aligned, `bytes`
+ * long, owned by the caller and never freed by the library) and the default policy mode.  *ctx (host)
+ * receives the handle.  DF_ERR_DEVICE without an sm_100 device. */
+int df_context_create(void* workspace, int64_t bytes, df_context** ctx);
+/* Frees the handle (not the workspace).  The caller synchronises its stream first. */
+int df_context_destroy(df_context* ctx);
+int df_context_set_policy_mode(df_context* ctx, int mode);
+/* The knobs of df_debug_set_gemm_flags, for this context. */
+int df_context_set_debug_flags(df_context* ctx, int flags);
+/* The entry points below with a context in front; same arguments, same results (bit for bit). */
+int df_context_emul_gemm(df_context* ctx, const double* A, const double* B, double* C,
+                         int64_t m, int64_t n, int64_t k, double tol, void* stream);
+int df_context_emul_gemm_slices(df_context* ctx, const double* A, const double* B, double* C,
+                                int64_t m, int64_t n, int64_t k, int s, void* stream);
+int df_context_jk_build(df_context* ctx, const double* B_packed, int64_t nao, int64_t naux,
+                        const double* C_occ, int64_t nocc, const double* D,
+                        double tol, double* J, double* K, void* stream);
+int df_context_jk_build_slices(df_context* ctx, const double* B_packed, int64_t nao, int64_t naux,
+                               const double* C_occ, int64_t nocc, const double* D,
+                               int s, double* J, double* K, void* stream);
+int df_context_jk_plan_create(df_context* ctx, const double* B_packed, int64_t nao, int64_t naux, int smax,
+                              void* plan, int64_t plan_bytes, void* stream);
+int df_context_jk_build_planned(df_context* ctx, const void* plan, int smax, const double* B_packed,
+                                int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
+                                const double* D, double tol, double* J, double* K, void* stream);
+int df_context_jk_build_planned_slices(df_context* ctx, const void* plan, int smax, const double* B_packed,
+                                       int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
+                                       const double* D, int s, double* J, double* K, void* stream);
+int df_context_last_status(df_context* ctx, void* stream, int* status);
+
+/* ---- the two mandated entry points (default context) --------------------- */
 
 /* C = A . B emulated with s = df_slices_for_tol(tol) INT8 slices.
  * A: m x k, B: k x n, C: m x n, all FP64 row-major, device.  C is overwritten.
@@ -204,7 +242,8 @@ int df_debug_set_gemm_flags(int flags);
 /* Number of GPU kernels this library has launched in this process. */
 int64_t df_launch_count(void);
 
-/* Per-kernel-class device timing for the roofline report (bench.py).  While
+/* Per-kernel-class device timing for the roofline report (bench.py); process-wide, for one stream at a
+ * time (do not enable it while several contexts run concurrently).  While
  * enabled, every entry point brackets each kernel class it launches with a pair
  * of CUDA events on the caller's stream.  df_profile_read() SYNCHRONISES on the
  * recorded events, returns the summed milliseconds and the number of brackets

@@ -9,7 +9,7 @@ been built, and DFError(DF_ERR_DEVICE) on a machine without an sm_100 GPU.
 import importlib
 
 _EXPORTS = (
-    "DFError", "Workspace", "Plan", "EXPORTS", "lib", "lib_path",
+    "DFError", "Workspace", "Context", "Plan", "EXPORTS", "lib", "lib_path",
     "DF_MODE_NOMINAL", "DF_MODE_GUARDED", "DF_STATUS_NONFINITE", "DF_STATUS_RANGE",
     "df_slices_for_tol", "df_num_int8_gemms", "df_kflush", "df_set_policy_mode", "df_plane_pitch",
     "df_emul_gemm_workspace_bytes", "df_jk_workspace_bytes", "df_jk_workspace_bytes_blocks", "df_set_workspace",

@@ -56,6 +56,18 @@ _SIG = {
     "df_jk_build_planned": (_i32, [_vp, _i32, _vp, _i64, _i64, _vp, _i64, _vp, _f64, _vp, _vp, _vp]),
     "df_jk_build_planned_slices": (_i32, [_vp, _i32, _vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
     "df_last_status": (_i32, [_vp, C.POINTER(C.c_int)]),
+    "df_context_create": (_i32, [_vp, _i64, C.POINTER(_vp)]),
+    "df_context_destroy": (_i32, [_vp]),
+    "df_context_set_policy_mode": (_i32, [_vp, _i32]),
+    "df_context_set_debug_flags": (_i32, [_vp, _i32]),
+    "df_context_emul_gemm": (_i32, [_vp, _vp, _vp, _vp, _i64, _i64, _i64, _f64, _vp]),
+    "df_context_emul_gemm_slices": (_i32, [_vp, _vp, _vp, _vp, _i64, _i64, _i64, _i32, _vp]),
+    "df_context_jk_build": (_i32, [_vp, _vp, _i64, _i64, _vp, _i64, _vp, _f64, _vp, _vp, _vp]),
+    "df_context_jk_build_slices": (_i32, [_vp, _vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
+    "df_context_jk_plan_create": (_i32, [_vp, _vp, _i64, _i64, _i32, _vp, _i64, _vp]),
+    "df_context_jk_build_planned": (_i32, [_vp, _vp, _i32, _vp, _i64, _i64, _vp, _i64, _vp, _f64, _vp, _vp, _vp]),
+    "df_context_jk_build_planned_slices": (_i32, [_vp, _vp, _i32, _vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
+    "df_context_last_status": (_i32, [_vp, _vp, C.POINTER(C.c_int)]),
     "df_debug_split_rows": (_i32, [_vp, _i64, _i64, _i32, _vp, _vp, _vp]),
     "df_debug_split_cols": (_i32, [_vp, _i64, _i64, _i32, _vp, _vp, _vp]),
     "df_debug_weight_sums": (_i32, [_vp, _vp, _i64, _i64, _i64, _i32, _i32, _i32, _vp, _vp]),
@@ -155,6 +167,91 @@ class Workspace:
     def close(self):
         df_set_workspace(None)
         self.buf = self.view = None
+
+
+class Context:
+    """A df_context: owns a device buffer as its workspace.  One context per concurrent stream; the
+    methods have the names and argument order of the df_context_* entry points (marshalling only)."""
+
+    def __init__(self, nbytes: int, device="cuda"):
+        import torch
+
+        self.buf = torch.empty(int(nbytes) + 256, dtype=torch.uint8, device=device)
+        off = (-self.buf.data_ptr()) % 256
+        self.view = self.buf[off: off + int(nbytes)]
+        h = _vp()
+        with torch.cuda.device(self.buf.device):
+            _check(lib.df_context_create(_ptr(self.view), int(nbytes), C.byref(h)), "df_context_create")
+        self.handle = h
+
+    def close(self):
+        if self.handle is not None:
+            _check(lib.df_context_destroy(self.handle), "df_context_destroy")
+        self.handle = self.buf = self.view = None
+
+    def set_policy_mode(self, mode: int) -> None:
+        _check(lib.df_context_set_policy_mode(self.handle, int(mode)), "df_context_set_policy_mode")
+
+    def set_debug_flags(self, flags: int) -> None:
+        _check(lib.df_context_set_debug_flags(self.handle, int(flags)), "df_context_set_debug_flags")
+
+    def emul_gemm(self, A, B, Cout, m, n, k, tol, stream=None) -> None:
+        import torch
+
+        f = torch.float64
+        _check(lib.df_context_emul_gemm(self.handle, _ptr(A, f), _ptr(B, f), _ptr(Cout, f), m, n, k, float(tol),
+                                        _stream(stream)), "df_context_emul_gemm")
+
+    def emul_gemm_slices(self, A, B, Cout, m, n, k, s, stream=None) -> None:
+        import torch
+
+        f = torch.float64
+        _check(lib.df_context_emul_gemm_slices(self.handle, _ptr(A, f), _ptr(B, f), _ptr(Cout, f), m, n, k, int(s),
+                                               _stream(stream)), "df_context_emul_gemm_slices")
+
+    def jk_build(self, B_packed, nao, naux, C_occ, nocc, D, tol, J, K, stream=None) -> None:
+        import torch
+
+        f = torch.float64
+        _check(lib.df_context_jk_build(self.handle, _ptr(B_packed, f), nao, naux, _ptr(C_occ, f), nocc, _ptr(D, f),
+                                       float(tol), _ptr(J, f), _ptr(K, f), _stream(stream)), "df_context_jk_build")
+
+    def jk_build_slices(self, B_packed, nao, naux, C_occ, nocc, D, s, J, K, stream=None) -> None:
+        import torch
+
+        f = torch.float64
+        _check(lib.df_context_jk_build_slices(self.handle, _ptr(B_packed, f), nao, naux, _ptr(C_occ, f), nocc,
+                                              _ptr(D, f), int(s), _ptr(J, f), _ptr(K, f), _stream(stream)),
+               "df_context_jk_build_slices")
+
+    def jk_plan_create(self, B_packed, nao, naux, smax, plan_view, stream=None) -> None:
+        import torch
+
+        _check(lib.df_context_jk_plan_create(self.handle, _ptr(B_packed, torch.float64), nao, naux, int(smax),
+                                             _ptr(plan_view), plan_view.numel(), _stream(stream)),
+               "df_context_jk_plan_create")
+
+    def jk_build_planned(self, plan, B_packed, nao, naux, C_occ, nocc, D, tol, J, K, stream=None) -> None:
+        import torch
+
+        f = torch.float64
+        _check(lib.df_context_jk_build_planned(self.handle, _ptr(plan.view), plan.smax, _ptr(B_packed, f), nao, naux,
+                                               _ptr(C_occ, f), nocc, _ptr(D, f), float(tol), _ptr(J, f), _ptr(K, f),
+                                               _stream(stream)), "df_context_jk_build_planned")
+
+    def jk_build_planned_slices(self, plan, B_packed, nao, naux, C_occ, nocc, D, s, J, K, stream=None) -> None:
+        import torch
+
+        f = torch.float64
+        _check(lib.df_context_jk_build_planned_slices(self.handle, _ptr(plan.view), plan.smax, _ptr(B_packed, f), nao,
+                                                      naux, _ptr(C_occ, f), nocc, _ptr(D, f), int(s), _ptr(J, f),
+                                                      _ptr(K, f), _stream(stream)),
+               "df_context_jk_build_planned_slices")
+
+    def last_status(self, stream=None) -> int:
+        out = C.c_int(0)
+        _check(lib.df_context_last_status(self.handle, _stream(stream), C.byref(out)), "df_context_last_status")
+        return int(out.value)
 
 
 # ---- the two entry points -----------------------------------------------------------------

@@ -16,14 +16,28 @@ namespace dfe {
 static std::atomic<long long> g_launches{0};
 void count_launch(int n) { g_launches += n; }
 
-static void* g_ws = nullptr;
-static int64_t g_ws_bytes = 0;
-static int g_mode = DF_MODE_GUARDED;
-static int g_device_ok = -1;
-static int g_g5_split_n = 1;
-static int g_g5_cluster = 1;
-static int g_wide_n = 1;
-static int g_g5_pair_halves = 1;
+}  // namespace dfe
+
+// A context: one workspace, one device, its policy mode, debug knobs and tensor-map cache.  One
+// context serves one stream at a time; two contexts (two workspaces) may run concurrently.  The entry
+// points without a context argument use the process-wide default context (df_set_workspace).
+struct df_context {
+  void* ws = nullptr;
+  int64_t ws_bytes = 0;
+  int device = -1;  // the device the workspace was registered on
+  int mode = DF_MODE_GUARDED;
+  dfe::LaunchEnv env;
+  // knobs decoded from env.flags (include/df_emul.h, df_debug_set_gemm_flags)
+  bool g5_split_n() const { return !(env.flags & 4); }            // bit 2: GEMM(5) keeps one N tile
+  bool g5_cluster() const { return !(env.flags & 64); }           // bit 6: N halves without the multicast pair
+  bool wide_n() const { return !((env.flags >> 24) & 1); }        // bit 24: df_emul_gemm never takes wide tiles
+  bool g5_pair_halves() const { return !((env.flags >> 22) & 1); }  // bit 22: N halves never on MMA pairs
+  int jk_dbg() const { return (env.flags >> 4) & 3; }             // bits 4, 5: unpack kernel without stores / loads
+};
+
+namespace dfe {
+
+static df_context g_default;
 
 // ---- optional per-kernel-class CUDA-event timing (df_profile_*; bench.py's roofline) ----
 enum ProfClass { kPSplit = 0, kPPassA, kPJGemv, kPUnpack, kPGemm5, kPSplitX, kPGemm6, kPReduce, kPGemm, kPNum };
@@ -66,17 +80,47 @@ struct ProfScope {
   }
 };
 
-static int device_ok() {
-  if (g_device_ok < 0) {
-    int dev = 0;
-    cudaDeviceProp prop;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
-      cudaGetLastError();
-      return 0;  // not cached: a later call may find a device
-    }
-    g_device_ok = (prop.major == 10) ? 1 : 0;
+// The current device when it is of compute capability 10.x, else -1.
+static int current_sm100_device(int* num_sms = nullptr) {
+  int dev = 0, major = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return -1;
   }
-  return g_device_ok;
+  if (major != 10) return -1;
+  if (num_sms) cudaDeviceGetAttribute(num_sms, cudaDevAttrMultiProcessorCount, dev);
+  return dev;
+}
+
+// DF_OK when the context has a workspace and the current device is the one it was registered on.
+static int context_ready(const df_context& c) {
+  const int dev = current_sm100_device();
+  if (dev < 0) return DF_ERR_DEVICE;
+  if (!c.ws) return DF_ERR_WORKSPACE;
+  if (dev != c.device) return DF_ERR_DEVICE;
+  return DF_OK;
+}
+
+static int context_set_workspace(df_context& c, void* ptr, int64_t bytes) {
+  if (!ptr || bytes <= 0) {
+    c.ws = nullptr;
+    c.ws_bytes = 0;
+    c.device = -1;
+    return DF_OK;
+  }
+  if (((uintptr_t)ptr & 255) != 0) return DF_ERR_ALIGN;
+  if (bytes < 256) return DF_ERR_WORKSPACE;
+  int num_sms = 0;
+  const int dev = current_sm100_device(&num_sms);
+  if (dev < 0) return DF_ERR_DEVICE;
+  if (cudaMemset(ptr, 0, 256) != cudaSuccess) return DF_ERR_CUDA;  // the status word
+  c.ws = ptr;
+  c.ws_bytes = bytes;
+  c.device = dev;
+  c.env.num_sms = num_sms;
+  if (!c.env.tmaps) c.env.tmaps = tmap_cache_create();
+  return DF_OK;
 }
 
 static int slices_for_tol(double tol, int mode) {
@@ -137,16 +181,15 @@ static GemmWs carve_gemm(void* base, int64_t m, int64_t n, int64_t k, int s) {
   return w;
 }
 
-static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, int s,
-                          cudaStream_t st) {
+static int emul_gemm_impl(df_context& c, const double* A, const double* B, double* C, int64_t m, int64_t n,
+                          int64_t k, int s, cudaStream_t st) {
   if (!A || !B || !C) return DF_ERR_NULL;
   // n: the column split puts 32-column blocks on grid.y (65535)
   if (m <= 0 || n <= 0 || k <= 0 || k > (1ll << 30) || m >= (1ll << 31) || n > 65535ll * 32) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
-  if (!device_ok()) return DF_ERR_DEVICE;
-  if (!g_ws) return DF_ERR_WORKSPACE;
-  GemmWs w = carve_gemm(g_ws, m, n, k, s);
-  if (w.bytes > g_ws_bytes) return DF_ERR_WORKSPACE;
+  if (const int rc = context_ready(c)) return rc;
+  GemmWs w = carve_gemm(c.ws, m, n, k, s);
+  if (w.bytes > c.ws_bytes) return DF_ERR_WORKSPACE;
 
   {
     ProfScope ps(kPSplit, st);
@@ -168,7 +211,7 @@ static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m
   g.s = s;
   // 256-column tiles when all s accumulators still fit TMEM (s <= 2): one or three MMAs per K step
   // are fed by 2 s plane tiles, so the operand feed, not the tensor pipe, bounds s = 1, 2
-  g.n_tile = n > 128 ? ((s <= 2 && n >= 256 && g_wide_n) ? 256 : (s == 3 && n >= 160 && g_wide_n) ? 160 : 128) : pad16(n);
+  g.n_tile = n > 128 ? ((s <= 2 && n >= 256 && c.wide_n()) ? 256 : (s == 3 && n >= 160 && c.wide_n()) ? 160 : 128) : pad16(n);
   g.bk = 0;
   g.nz = 1;
   g.zk = nullptr;
@@ -180,7 +223,7 @@ static int emul_gemm_impl(const double* A, const double* B, double* C, int64_t m
   g.ldc = n;
   {
     ProfScope ps(kPGemm, st);
-    if (launch_gemm_i8(g, st) != cudaSuccess) return DF_ERR_CUDA;
+    if (launch_gemm_i8(g, c.env, st) != cudaSuccess) return DF_ERR_CUDA;
   }
   return DF_OK;
 }
@@ -277,8 +320,8 @@ __global__ void jk_group_tables_kernel(int nq, GroupGeom gg, int ng, int* qgroup
 }
 
 // plan != nullptr (with its slice count smax): a planned build, GEMM(5) reads the plan's planes.
-static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Cocc, int64_t nocc, const double* D,
-                   int s, double* J, double* K, double* X_out, int32_t* e6_out, int* ngroups_out,
+static int jk_impl(df_context& c, const double* Bp, int64_t nao, int64_t naux, const double* Cocc, int64_t nocc,
+                   const double* D, int s, double* J, double* K, double* X_out, int32_t* e6_out, int* ngroups_out,
                    cudaStream_t st, const void* plan = nullptr, int smax = 0) {
   if (!Bp || !Cocc || !D || !J || !K) return DF_ERR_NULL;
   const bool planned = plan != nullptr;
@@ -286,8 +329,7 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
   if (planned && ((uintptr_t)plan & 255) != 0) return DF_ERR_ALIGN;
   if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nao > 11552 || naux > (1 << 20)) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
-  if (!device_ok()) return DF_ERR_DEVICE;
-  if (!g_ws) return DF_ERR_WORKSPACE;
+  if (const int rc = context_ready(c)) return rc;
   // largest super-block (multiple of 512 q, capped so that GEMM(6)'s contraction offsets and the
   // row count of GEMM(5) stay in int32) that fits the workspace
   int64_t QS = 0;
@@ -296,14 +338,14 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     for (int64_t nb = nblk; nb >= 1; --nb) {
       const int64_t qs = (nb == nblk) ? naux : nb * kQBlock;
       if (qs * pad16(nocc) >= (1ll << 30) || qs * nao >= (1ll << 31) - 256) continue;
-      if (carve_jk(nullptr, nao, naux, nocc, s, qs, planned).bytes <= g_ws_bytes) {
+      if (carve_jk(nullptr, nao, naux, nocc, s, qs, planned).bytes <= c.ws_bytes) {
         QS = qs;
         break;
       }
     }
   }
   if (QS == 0) return DF_ERR_WORKSPACE;
-  JkWs w = carve_jk(g_ws, nao, naux, nocc, s, QS, planned);
+  JkWs w = carve_jk(c.ws, nao, naux, nocc, s, QS, planned);
   const PlanLayout PL = plan_layout(nao, naux, planned ? smax : 1);
   const char* const plan_b = static_cast<const char*>(plan);
   const int64_t npair = nao * (nao + 1) / 2;
@@ -353,7 +395,7 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
       ProfScope ps(kPUnpack, st);
       DFE_CK(launch_jk_unpack_split(Bp, (int)nao, (int)naux, (int)qs0, (int)qs1, w.emax5, s, w.e5, w.p5,
                                     w.pitchj, (int64_t)nq * nao * w.pitchj, w.status, w.rho,
-                                    w.jpart + (qs0 / 32) * npair, st));
+                                    w.jpart + (qs0 / 32) * npair, c.jk_dbg(), st));
     }
     if (!planned && qs1 == naux) {
       ProfScope ps(kPJGemv, st);
@@ -378,23 +420,23 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     g5.n_tile = w.a_pad;
     {
       const int W0 = 512 / (int)round_up(w.a_pad, 32);
-      if (s == W0 + 1 && W0 >= 3 && w.a_pad % 32 == 0 && g_g5_split_n) {
+      if (s == W0 + 1 && W0 >= 3 && w.a_pad % 32 == 0 && c.g5_split_n()) {
         // one more weight than TMEM slots: the whole a_pad on cta_group::2 pairs, second pass (one
         // weight) with the running sum parked in TMEM -- 9.3-10.5 ms at nocc = 150, s = 4, against
         // 10.8-11.5 ms for two single-pass halves on MMA pairs (A streamed twice)
         g5.pair = 1;
-      } else if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && g_g5_split_n) {
+      } else if ((int64_t)s * round_up(w.a_pad, 32) > 512 && w.a_pad % 32 == 0 && c.g5_split_n()) {
         g5.n_tile = w.a_pad / 2;
         // one pass per half (all s accumulators in TMEM): the halves run as 256-row tiles on MMA pairs
         // (an MMA costs at least ~50 cycles per 128 rows whatever N, and a pair instruction covers
         // 256) -- 13.6 / 17.6 ms against 14.6 / 21.9 ms at s = 5 / 6 for the multicast pair below;
         // with several passes (s >= 7 at nocc = 150) the two are equal
-        if (g_g5_pair_halves && (int64_t)s * g5.n_tile <= 512) g5.pair = 1;
+        if (c.g5_pair_halves() && (int64_t)s * g5.n_tile <= 512) g5.pair = 1;
       }
     }
     g5.acc_stride = (g5.n_tile % 32) ? g5.n_tile : 0;
     g5.x_cols = w.a_pad;
-    g5.cluster_n = (g_g5_cluster && g5.n_tile * 2 == w.a_pad && !g5.pair) ? 2 : 1;
+    g5.cluster_n = (c.g5_cluster() && g5.n_tile * 2 == w.a_pad && !g5.pair) ? 2 : 1;
     g5.nz = 1;
     g5.eA = planned ? reinterpret_cast<const int32_t*>(plan_b + PL.e5_off) + qs0 * nao : w.e5;
     g5.eB = w.eC;
@@ -406,7 +448,7 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     g5.xmax = w.xmax;
       {
       ProfScope ps(kPGemm5, st);
-      DFE_CK(launch_gemm_i8(g5, st));
+      DFE_CK(launch_gemm_i8(g5, c.env, st));
     }
     if (X_out)
       DFE_CK(cudaMemcpyAsync(X_out + qs0 * nao * w.a_pad, w.X, sizeof(double) * nq * nao * w.a_pad,
@@ -445,7 +487,7 @@ static int jk_impl(const double* Bp, int64_t nao, int64_t naux, const double* Co
     g6.c_stride = nao * nao;
     {
       ProfScope ps(kPGemm6, st);
-      DFE_CK(launch_gemm_i8(g6, st));
+      DFE_CK(launch_gemm_i8(g6, c.env, st));
     }
     // H7: K += sum_g K_g in increasing-q order, mirrored to the upper triangle
     {
@@ -477,12 +519,6 @@ int df_num_int8_gemms(int s) { return (s < 1 || s > kMaxSlices) ? DF_ERR_TOL : s
 
 int df_kflush(int s) { return (s < 1 || s > kMaxSlices) ? DF_ERR_TOL : kflush_for(s); }
 
-int df_set_policy_mode(int mode) {
-  if (mode != DF_MODE_NOMINAL && mode != DF_MODE_GUARDED) return DF_ERR_TOL;
-  g_mode = mode;
-  return DF_OK;
-}
-
 int64_t df_plane_pitch(int64_t cols) { return cols <= 0 ? DF_ERR_DIM : plane_pitch(cols); }
 
 int64_t df_emul_gemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int s) {
@@ -506,43 +542,12 @@ int64_t df_jk_workspace_bytes_blocks(int64_t nao, int64_t naux, int64_t nocc, in
   return carve_jk(nullptr, nao, naux, nocc, s, qs).bytes;
 }
 
-int df_set_workspace(void* ptr, int64_t bytes) {
-  if (!ptr || bytes <= 0) {
-    g_ws = nullptr;
-    g_ws_bytes = 0;
-    return DF_OK;
-  }
-  if (((uintptr_t)ptr & 255) != 0) return DF_ERR_ALIGN;
-  if (bytes < 256) return DF_ERR_WORKSPACE;
-  if (!device_ok()) return DF_ERR_DEVICE;
-  if (cudaMemset(ptr, 0, 256) != cudaSuccess) return DF_ERR_CUDA;  // the status word
-  g_ws = ptr;
-  g_ws_bytes = bytes;
-  return DF_OK;
-}
-
-int df_emul_gemm(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, double tol,
-                 void* stream) {
-  const int s = slices_for_tol(tol, g_mode);
-  if (s < 0) return s;
-  return emul_gemm_impl(A, B, C, m, n, k, s, (cudaStream_t)stream);
-}
-
-int df_emul_gemm_slices(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, int s,
-                        void* stream) {
-  return emul_gemm_impl(A, B, C, m, n, k, s, (cudaStream_t)stream);
-}
-
-int df_jk_build(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
-                const double* D, double tol, double* J, double* K, void* stream) {
-  const int s = slices_for_tol(tol, g_mode);
-  if (s < 0) return s;
-  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream);
-}
-
-int df_jk_build_slices(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
-                       const double* D, int s, double* J, double* K, void* stream) {
-  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream);
+int64_t df_jk_planned_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, int s, int64_t nblocks) {
+  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nblocks < 1) return DF_ERR_DIM;
+  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
+  int64_t qs = nblocks * kQBlock;
+  if (qs > naux) qs = naux;
+  return carve_jk(nullptr, nao, naux, nocc, s, qs, true).bytes;
 }
 
 int64_t df_jk_plan_bytes(int64_t nao, int64_t naux, int smax) {
@@ -551,14 +556,77 @@ int64_t df_jk_plan_bytes(int64_t nao, int64_t naux, int smax) {
   return plan_layout(nao, naux, smax).bytes;
 }
 
-int df_jk_plan_create(const double* B_packed, int64_t nao, int64_t naux, int smax, void* plan, int64_t plan_bytes,
-                      void* stream) {
-  if (!B_packed || !plan) return DF_ERR_NULL;
+// ---- contexts -------------------------------------------------------------------------------
+
+int df_context_create(void* workspace, int64_t bytes, df_context** ctx) {
+  if (!ctx || !workspace) return DF_ERR_NULL;
+  df_context* c = new df_context();
+  const int rc = context_set_workspace(*c, workspace, bytes);
+  if (rc != DF_OK) {
+    delete c;
+    return rc;
+  }
+  *ctx = c;
+  return DF_OK;
+}
+
+int df_context_destroy(df_context* ctx) {
+  if (!ctx) return DF_ERR_NULL;
+  if (ctx == &g_default) return DF_ERR_NULL;
+  tmap_cache_destroy(ctx->env.tmaps);
+  delete ctx;
+  return DF_OK;
+}
+
+int df_context_set_policy_mode(df_context* ctx, int mode) {
+  if (!ctx) return DF_ERR_NULL;
+  if (mode != DF_MODE_NOMINAL && mode != DF_MODE_GUARDED) return DF_ERR_TOL;
+  ctx->mode = mode;
+  return DF_OK;
+}
+
+int df_context_set_debug_flags(df_context* ctx, int flags) {
+  if (!ctx) return DF_ERR_NULL;
+  ctx->env.flags = flags;
+  return DF_OK;
+}
+
+int df_context_emul_gemm(df_context* ctx, const double* A, const double* B, double* C, int64_t m, int64_t n,
+                         int64_t k, double tol, void* stream) {
+  if (!ctx) return DF_ERR_NULL;
+  const int s = slices_for_tol(tol, ctx->mode);
+  if (s < 0) return s;
+  return emul_gemm_impl(*ctx, A, B, C, m, n, k, s, (cudaStream_t)stream);
+}
+
+int df_context_emul_gemm_slices(df_context* ctx, const double* A, const double* B, double* C, int64_t m, int64_t n,
+                                int64_t k, int s, void* stream) {
+  if (!ctx) return DF_ERR_NULL;
+  return emul_gemm_impl(*ctx, A, B, C, m, n, k, s, (cudaStream_t)stream);
+}
+
+int df_context_jk_build(df_context* ctx, const double* B_packed, int64_t nao, int64_t naux, const double* C_occ,
+                        int64_t nocc, const double* D, double tol, double* J, double* K, void* stream) {
+  if (!ctx) return DF_ERR_NULL;
+  const int s = slices_for_tol(tol, ctx->mode);
+  if (s < 0) return s;
+  return jk_impl(*ctx, B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+int df_context_jk_build_slices(df_context* ctx, const double* B_packed, int64_t nao, int64_t naux,
+                               const double* C_occ, int64_t nocc, const double* D, int s, double* J, double* K,
+                               void* stream) {
+  if (!ctx) return DF_ERR_NULL;
+  return jk_impl(*ctx, B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+int df_context_jk_plan_create(df_context* ctx, const double* B_packed, int64_t nao, int64_t naux, int smax,
+                              void* plan, int64_t plan_bytes, void* stream) {
+  if (!ctx || !B_packed || !plan) return DF_ERR_NULL;
   if (nao <= 0 || naux <= 0 || nao > 11552 || naux > (1 << 20)) return DF_ERR_DIM;
   if (smax < 1 || smax > kMaxSlices) return DF_ERR_TOL;
   if (((uintptr_t)plan & 255) != 0) return DF_ERR_ALIGN;
-  if (!device_ok()) return DF_ERR_DEVICE;
-  if (!g_ws) return DF_ERR_WORKSPACE;  // the status word
+  if (const int rc = context_ready(*ctx)) return rc;  // the workspace holds the status word
   const PlanLayout L = plan_layout(nao, naux, smax);
   if (plan_bytes < L.bytes) return DF_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
@@ -575,63 +643,103 @@ int df_jk_plan_create(const double* B_packed, int64_t nao, int64_t naux, int sma
     if (launch_jk_unpack_split(B_packed, (int)nao, (int)naux, 0, (int)naux, emax, smax,
                                reinterpret_cast<int32_t*>(pb + L.e5_off),
                                reinterpret_cast<int8_t*>(pb + L.planes_off), L.pitch, L.plane_stride,
-                               (int*)g_ws, nullptr, nullptr, st) != cudaSuccess)
+                               (int*)ctx->ws, nullptr, nullptr, ctx->jk_dbg(), st) != cudaSuccess)
       return DF_ERR_CUDA;
   }
   return DF_OK;
 }
 
-int64_t df_jk_planned_workspace_bytes(int64_t nao, int64_t naux, int64_t nocc, int s, int64_t nblocks) {
-  if (nao <= 0 || naux <= 0 || nocc <= 0 || nocc > 256 || nblocks < 1) return DF_ERR_DIM;
-  if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
-  int64_t qs = nblocks * kQBlock;
-  if (qs > naux) qs = naux;
-  return carve_jk(nullptr, nao, naux, nocc, s, qs, true).bytes;
+int df_context_jk_build_planned(df_context* ctx, const void* plan, int smax, const double* B_packed, int64_t nao,
+                                int64_t naux, const double* C_occ, int64_t nocc, const double* D, double tol,
+                                double* J, double* K, void* stream) {
+  if (!ctx || !plan) return DF_ERR_NULL;
+  const int s = slices_for_tol(tol, ctx->mode);
+  if (s < 0) return s;
+  return jk_impl(*ctx, B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr,
+                 (cudaStream_t)stream, plan, smax);
+}
+
+int df_context_jk_build_planned_slices(df_context* ctx, const void* plan, int smax, const double* B_packed,
+                                       int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
+                                       const double* D, int s, double* J, double* K, void* stream) {
+  if (!ctx || !plan) return DF_ERR_NULL;
+  return jk_impl(*ctx, B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr,
+                 (cudaStream_t)stream, plan, smax);
+}
+
+int df_context_last_status(df_context* ctx, void* stream, int* status) {
+  if (!ctx || !status) return DF_ERR_NULL;
+  if (!ctx->ws) return DF_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (cudaMemcpyAsync(status, ctx->ws, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return DF_ERR_CUDA;
+  if (cudaMemsetAsync(ctx->ws, 0, sizeof(int), st) != cudaSuccess) return DF_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return DF_ERR_CUDA;
+  return DF_OK;
+}
+
+// ---- the same calls on the process-wide default context ------------------------------------
+
+int df_set_policy_mode(int mode) { return df_context_set_policy_mode(&g_default, mode); }
+
+int df_set_workspace(void* ptr, int64_t bytes) { return context_set_workspace(g_default, ptr, bytes); }
+
+int df_emul_gemm(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, double tol,
+                 void* stream) {
+  return df_context_emul_gemm(&g_default, A, B, C, m, n, k, tol, stream);
+}
+
+int df_emul_gemm_slices(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, int s,
+                        void* stream) {
+  return df_context_emul_gemm_slices(&g_default, A, B, C, m, n, k, s, stream);
+}
+
+int df_jk_build(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
+                const double* D, double tol, double* J, double* K, void* stream) {
+  return df_context_jk_build(&g_default, B_packed, nao, naux, C_occ, nocc, D, tol, J, K, stream);
+}
+
+int df_jk_build_slices(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
+                       const double* D, int s, double* J, double* K, void* stream) {
+  return df_context_jk_build_slices(&g_default, B_packed, nao, naux, C_occ, nocc, D, s, J, K, stream);
+}
+
+int df_jk_plan_create(const double* B_packed, int64_t nao, int64_t naux, int smax, void* plan, int64_t plan_bytes,
+                      void* stream) {
+  return df_context_jk_plan_create(&g_default, B_packed, nao, naux, smax, plan, plan_bytes, stream);
 }
 
 int df_jk_build_planned(const void* plan, int smax, const double* B_packed, int64_t nao, int64_t naux,
                         const double* C_occ, int64_t nocc, const double* D, double tol, double* J, double* K,
                         void* stream) {
-  if (!plan) return DF_ERR_NULL;
-  const int s = slices_for_tol(tol, g_mode);
-  if (s < 0) return s;
-  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream,
-                 plan, smax);
+  return df_context_jk_build_planned(&g_default, plan, smax, B_packed, nao, naux, C_occ, nocc, D, tol, J, K, stream);
 }
 
 int df_jk_build_planned_slices(const void* plan, int smax, const double* B_packed, int64_t nao, int64_t naux,
                                const double* C_occ, int64_t nocc, const double* D, int s, double* J, double* K,
                                void* stream) {
-  if (!plan) return DF_ERR_NULL;
-  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, nullptr, nullptr, nullptr, (cudaStream_t)stream,
-                 plan, smax);
+  return df_context_jk_build_planned_slices(&g_default, plan, smax, B_packed, nao, naux, C_occ, nocc, D, s, J, K,
+                                            stream);
 }
+
+int df_last_status(void* stream, int* status) { return df_context_last_status(&g_default, stream, status); }
+
+// ---- debug exports (default context) --------------------------------------------------------
 
 int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
                       const double* D, int s, double* J, double* K, double* X_out, int32_t* e6_out,
                       int* ngroups_out, void* stream) {
-  return jk_impl(B_packed, nao, naux, C_occ, nocc, D, s, J, K, X_out, e6_out, ngroups_out, (cudaStream_t)stream);
-}
-
-int df_last_status(void* stream, int* status) {
-  if (!status) return DF_ERR_NULL;
-  if (!g_ws) return DF_ERR_WORKSPACE;
-  cudaStream_t st = (cudaStream_t)stream;
-  if (cudaMemcpyAsync(status, g_ws, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return DF_ERR_CUDA;
-  if (cudaMemsetAsync(g_ws, 0, sizeof(int), st) != cudaSuccess) return DF_ERR_CUDA;
-  if (cudaStreamSynchronize(st) != cudaSuccess) return DF_ERR_CUDA;
-  return DF_OK;
+  return jk_impl(g_default, B_packed, nao, naux, C_occ, nocc, D, s, J, K, X_out, e6_out, ngroups_out,
+                 (cudaStream_t)stream);
 }
 
 int df_debug_split_rows(const double* X, int64_t rows, int64_t cols, int s, int32_t* e, int8_t* planes,
                         void* stream) {
   if (!X || !e || !planes) return DF_ERR_NULL;
-  if (rows <= 0 || cols <= 0) return DF_ERR_DIM;
+  if (rows <= 0 || cols <= 0 || rows >= (1ll << 31)) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
-  if (!device_ok()) return DF_ERR_DEVICE;
-  if (!g_ws) return DF_ERR_WORKSPACE;
+  if (const int rc = context_ready(g_default)) return rc;
   const int64_t pitch = plane_pitch(cols);
-  if (launch_split_rows(X, rows, cols, cols, s, e, planes, pitch, rows * pitch, (int*)g_ws,
+  if (launch_split_rows(X, rows, cols, cols, s, e, planes, pitch, rows * pitch, (int*)g_default.ws,
                         (cudaStream_t)stream) != cudaSuccess)
     return DF_ERR_CUDA;
   return DF_OK;
@@ -641,11 +749,11 @@ int df_debug_split_cols(const double* X, int64_t k, int64_t n, int s, int32_t* e
   if (!X || !e || !planes) return DF_ERR_NULL;
   if (k <= 0 || n <= 0 || k > (1ll << 30) || n > 65535ll * 32) return DF_ERR_DIM;
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
-  if (!device_ok()) return DF_ERR_DEVICE;
-  if (!g_ws || g_ws_bytes < 256 + round_up(4 * n, 256)) return DF_ERR_WORKSPACE;
+  if (const int rc = context_ready(g_default)) return rc;
+  if (g_default.ws_bytes < 256 + round_up(4 * n, 256)) return DF_ERR_WORKSPACE;
   const int64_t pitch = plane_pitch(k);
-  uint32_t* cmax = (uint32_t*)((char*)g_ws + 256);
-  if (launch_split_cols(X, k, n, s, cmax, e, planes, pitch, n * pitch, (int*)g_ws, (cudaStream_t)stream) !=
+  uint32_t* cmax = (uint32_t*)((char*)g_default.ws + 256);
+  if (launch_split_cols(X, k, n, s, cmax, e, planes, pitch, n * pitch, (int*)g_default.ws, (cudaStream_t)stream) !=
       cudaSuccess)
     return DF_ERR_CUDA;
   return DF_OK;
@@ -658,7 +766,7 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t 
   if (s < 1 || s > kMaxSlices) return DF_ERR_TOL;
   if (bk != 0 && bk != 32 && bk != 64 && bk != 128) return DF_ERR_DIM;
   if (chunk < 0 || (int64_t)chunk * kflush_for(s) >= k) return DF_ERR_DIM;
-  if (!device_ok()) return DF_ERR_DEVICE;
+  if (current_sm100_device() < 0) return DF_ERR_DEVICE;
   const int64_t pitch = plane_pitch(k);
   GemmProblem g = {};
   g.A = DA;
@@ -676,17 +784,14 @@ int df_debug_weight_sums(const int8_t* DA, const int8_t* DB, int64_t m, int64_t 
   g.mode = kEpiInt32;
   g.P = P;
   g.dbg_chunk = chunk;
-  if (launch_gemm_i8(g, (cudaStream_t)stream) != cudaSuccess) return DF_ERR_CUDA;
+  LaunchEnv env;  // no cache, the SM count of the current device
+  env.flags = g_default.env.flags;
+  if (launch_gemm_i8(g, env, (cudaStream_t)stream) != cudaSuccess) return DF_ERR_CUDA;
   return DF_OK;
 }
 
 int df_debug_set_gemm_flags(int flags) {
-  set_gemm_debug_flags(flags);
-  g_g5_split_n = (flags & 4) ? 0 : 1;  // bit 2: GEMM(5) keeps one N tile
-  g_g5_cluster = (flags & 64) ? 0 : 1;  // bit 6: GEMM(5) N halves without the multicast pair
-  set_jk_debug_flags((flags >> 4) & 3);
-  g_wide_n = ((flags >> 24) & 1) ? 0 : 1;  // bit 24: df_emul_gemm never takes 256-column tiles  // bits 4, 5: unpack kernel without stores / without loads
-  g_g5_pair_halves = ((flags >> 22) & 1) ? 0 : 1;  // bit 22: GEMM(5) N halves never on MMA pairs
+  g_default.env.flags = flags;
   set_peak_tiles((flags >> 16) & 15);  // bits 16-19: MMA probe operand tiles / swizzle
   return DF_OK;
 }
@@ -729,7 +834,7 @@ int df_debug_mma_peak(int n_mma, int iters, int grid, float* ms, void* stream) {
   if (n < 16 || n > 256 || (n % 16) != 0 || iters < 2 || grid < 1) return DF_ERR_DIM;
   if (nissue < 0 || nissue > 4 || 2 * (nissue ? nissue : 1) * n > 512) return DF_ERR_DIM;
   if (pairp && (nissue != 0 || grid < 2 || (n % 32) != 0)) return DF_ERR_DIM;
-  if (!device_ok()) return DF_ERR_DEVICE;
+  if (current_sm100_device() < 0) return DF_ERR_DEVICE;
   if (launch_mma_peak(n_mma, iters, grid, ms, (cudaStream_t)stream) != cudaSuccess) return DF_ERR_CUDA;
   return DF_OK;
 }

@@ -801,28 +801,60 @@ static uint32_t stage_stride_for(int s, int n_tile, int bk) {
   return (uint32_t)round_up((int64_t)s * (kTileM + n_tile) * bk, 1024);  // n_tile / 2 passed in pair mode
 }
 
-static int g_gemm_dbg_flags = 0;
-static int g_gemm_force_bk = 0;
-static int g_gemm_no_tp = 0;
-static int g_gemm_no_pair = 0;
-void set_gemm_debug_flags(int flags) {
-  g_gemm_dbg_flags = (flags & 3) | (((flags >> 23) & 1) << 2);  // bit 23: staged 16-byte epilogue accesses, no 256-bit ones
-  g_gemm_no_pair = (flags >> 20) & 1;  // bit 20: no cta_group::2 pair tiles
-  g_gemm_no_tp = (flags >> 3) & 1;  // bit 3: multi-pass through global read-modify-write instead of TMEM
-  const int f = (flags >> 8) & 0xFF;  // bits 8..15: force the K-block width (32, 64, 128; 0 = auto)
-  g_gemm_force_bk = (f == 32 || f == 64 || f == 128) ? f : 0;
+// Tensor maps of the GEMM operands, cached per context: a map depends only on the pointer, the shape
+// and the box, and a build of a small problem spends more host time encoding its maps (four driver
+// calls per GEMM launch) than launching the kernel.
+struct TmapKey {
+  const void* base;
+  int64_t k, rows, pitch, plane_stride;
+  int planes, bk, box_rows;
+  bool operator==(const TmapKey& o) const {
+    return base == o.base && k == o.k && rows == o.rows && pitch == o.pitch && plane_stride == o.plane_stride &&
+           planes == o.planes && bk == o.bk && box_rows == o.box_rows;
+  }
+};
+struct TmapCache {
+  static constexpr int kSlots = 48;
+  TmapKey keys[kSlots];
+  CUtensorMap maps[kSlots];
+  int used = 0, next = 0;
+};
+TmapCache* tmap_cache_create() { return new TmapCache(); }
+void tmap_cache_destroy(TmapCache* c) { delete c; }
+
+static bool cached_plane_map(TmapCache* cache, CUtensorMap* map, const int8_t* base, int64_t k, int64_t rows, int planes,
+                             int64_t pitch, int64_t plane_stride, int bk, int box_rows) {
+  if (!cache) return make_plane_map(map, base, k, rows, planes, pitch, plane_stride, bk, box_rows);
+  const TmapKey key = {base, k, rows, pitch, plane_stride, planes, bk, box_rows};
+  for (int i = 0; i < cache->used; ++i)
+    if (cache->keys[i] == key) {
+      *map = cache->maps[i];
+      return true;
+    }
+  if (!make_plane_map(map, base, k, rows, planes, pitch, plane_stride, bk, box_rows)) return false;
+  const int slot = cache->used < TmapCache::kSlots ? cache->used++ : (cache->next++ % TmapCache::kSlots);
+  cache->keys[slot] = key;
+  cache->maps[slot] = *map;
+  return true;
 }
 
-cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
+cudaError_t launch_gemm_i8(const GemmProblem& g, const LaunchEnv& env, cudaStream_t st) {
   GemmKernelParams p;
   const int s = g.s;
+  // debug knobs (include/df_emul.h, df_debug_set_gemm_flags)
+  const int flags = env.flags;
+  const int dbg_kernel = (flags & 3) | (((flags >> 23) & 1) << 2);  // bit 23: staged 16-byte epilogue accesses, no 256-bit ones
+  const bool no_pair = (flags >> 20) & 1;                           // bit 20: no cta_group::2 pair tiles
+  const bool no_tp = (flags >> 3) & 1;  // bit 3: multi-pass through global read-modify-write instead of TMEM
+  const int fbk = (flags >> 8) & 0xFF;  // bits 8..15: force the K-block width (32, 64, 128; 0 = auto)
+  const int force_bk = (fbk == 32 || fbk == 64 || fbk == 128) ? fbk : 0;
   // cta_group::2 pair: 256-row tiles on an SM pair, each CTA holds half of the B tile's N rows --
   // the MMA then reads 6 KB instead of 8 KB of shared memory per 128 x 128 x 32 step
   const bool pair = g.pair && g.n_tile % 16 == 0 && g.mode != kEpiInt32 && g.a_rows > kTileM &&
-                    (!g.lower_only || g.n_tile == 128) && !g_gemm_no_pair;
+                    (!g.lower_only || g.n_tile == 128) && !no_pair;
   const int nb = pair ? g.n_tile / 2 : g.n_tile;  // B rows per CTA and stage
   int bk = g.bk;
-  if (bk == 0) bk = g_gemm_force_bk;
+  if (bk == 0) bk = force_bk;
   if (bk == 0) {
     // widest swizzle span that still gives two stages (measured: 128-byte K blocks with two stages
     // beat 64-byte blocks with four: full 128-byte lines per TMA row and half the barrier traffic)
@@ -837,8 +869,8 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.num_stages = (int)((kSmemLimit - 1024) / p.stage_stride);
   if (p.num_stages > kMaxStages) p.num_stages = kMaxStages;
   if (p.num_stages < 1) return cudaErrorInvalidValue;
-  if (!make_plane_map(&p.mapA, g.A, g.k, g.a_rows, s, g.a_pitch, g.a_plane_stride, bk, kTileM) ||
-      !make_plane_map(&p.mapB, g.B, g.k, g.b_rows, s, g.b_pitch, g.b_plane_stride, bk, g.n_tile))
+  if (!cached_plane_map(env.tmaps, &p.mapA, g.A, g.k, g.a_rows, s, g.a_pitch, g.a_plane_stride, bk, kTileM) ||
+      !cached_plane_map(env.tmaps, &p.mapB, g.B, g.k, g.b_rows, s, g.b_pitch, g.b_plane_stride, bk, g.n_tile))
     return cudaErrorInvalidValue;
   p.s = s;
   p.n_tile = g.n_tile;
@@ -851,7 +883,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
     if (s <= W0) {
       p.weights_per_pass = s;
       p.npass = 1;
-    } else if (W0 >= 3 && one_chunk && g.mode != kEpiInt32 && !g_gemm_no_tp &&
+    } else if (W0 >= 3 && one_chunk && g.mode != kEpiInt32 && !no_tp &&
                1 + (s - W0 + W0 - 3) / (W0 - 2) <= (s + W0 - 1) / W0) {
       // park the running sum in TMEM when that costs no extra pass over the contraction
       p.tp = 1;
@@ -928,7 +960,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
   p.xmax = g.xmax;
   p.P = g.P;
   p.dbg_chunk = g.dbg_chunk;
-  p.dbg_flags = g_gemm_dbg_flags;
+  p.dbg_flags = dbg_kernel;
 
   p.pair = pair ? 1 : 0;
   const int tiles_m2 = (p.tiles_m + 1) / 2;  // 256-row tiles of the pair mode
@@ -936,12 +968,12 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
                        : (g.lower_only ? p.tiles_m * (p.tiles_m + 1) / 2 : p.tiles_m * p.tiles_n);
   if (pair) {
     p.tiles_m = tiles_m2;  // decode_work rasterises pair rows; the kernel maps them back to 2 tm2 + rank
-    if (!make_plane_map(&p.mapBh, g.B, g.k, g.b_rows, s, g.b_pitch, g.b_plane_stride, bk, g.n_tile / 2))
+    if (!cached_plane_map(env.tmaps, &p.mapBh, g.B, g.k, g.b_rows, s, g.b_pitch, g.b_plane_stride, bk, g.n_tile / 2))
       return cudaErrorInvalidValue;
   }
   p.total_work = (long long)p.tiles_per_z * g.nz;
-  static int num_sms = 0;
-  if (!num_sms) {
+  int num_sms = env.num_sms;
+  if (num_sms <= 0) {
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
@@ -952,7 +984,7 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st) {
                  : (g.cluster_n == 2 && p.tiles_n == 2 && !g.lower_only && num_sms >= 2) ? 2 : 1;
   if (cl == 2) {
     p.group_m = 1;  // work items 2c, 2c+1 = (tm = c, tn = 0 / 1)
-    if (!make_plane_map(&p.mapA2, g.A, g.k, g.a_rows, s, g.a_pitch, g.a_plane_stride, bk, 64)) return cudaErrorInvalidValue;
+    if (!cached_plane_map(env.tmaps, &p.mapA2, g.A, g.k, g.a_rows, s, g.a_pitch, g.a_plane_stride, bk, 64)) return cudaErrorInvalidValue;
   }
   // persistent when tiles are short (the per-CTA set-up of ~4 us would show); long-K tiles are left
   // to the hardware scheduler, which balances them better than a static round-robin

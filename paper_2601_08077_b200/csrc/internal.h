@@ -50,6 +50,16 @@ __host__ __device__ inline int group_col(const GroupGeom& g, int gi, int nq, int
   return (last / g.gpb) * g.wblock + (last % g.gpb) * g.wfull + (w + 31) / 32 * 32;
 }
 
+// What a launch needs beyond its problem; owned by a context (api.cu), one per concurrent stream.
+struct TmapCache;  // gemm_i8.cu: tensor maps of the GEMM operands, keyed by (pointer, shape, box)
+TmapCache* tmap_cache_create();
+void tmap_cache_destroy(TmapCache* c);
+struct LaunchEnv {
+  int num_sms = 0;
+  int flags = 0;               // df_debug_set_gemm_flags / df_context_set_debug_flags bits
+  TmapCache* tmaps = nullptr;  // may be null: every launch encodes its maps
+};
+
 // ---- tmap.cu ---------------------------------------------------------------
 // cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked).
 // dtype: 0 = UINT8, 1 = FLOAT64; swizzle: 0 (none), 32, 64, 128 bytes.  dims/box: rank entries,
@@ -110,12 +120,10 @@ struct GemmProblem {
   int dbg_chunk;
 };
 
-cudaError_t launch_gemm_i8(const GemmProblem& g, cudaStream_t st);
-void set_gemm_debug_flags(int flags);
+cudaError_t launch_gemm_i8(const GemmProblem& g, const LaunchEnv& env, cudaStream_t st);
 void set_peak_tiles(int n);  // probe walks n distinct operand tiles (1 = the same tile every MMA)
 cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStream_t st);
 
-void set_jk_debug_flags(int flags);  // timing experiments: bit 0 = unpack writes nothing, bit 1 = reads nothing
 // ---- jk.cu ----------------------------------------------------------------
 // pass A over packed B: rho[q] (through rho_part[jk_rho_part_rows(nao)][naux], every element of
 // which is written, summed in a fixed order) and emax[i * naux + q] = upper word of max_j |B^q_ij|
@@ -128,9 +136,10 @@ cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* 
 cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const double* rho, double* Jp,
                              cudaStream_t st);
 // unpack + split q in [q0, q1): planes5[t][(q - q0) * nao + i][pitch], e5[(q - q0) * nao + i]
+// dbg (timing experiments): bit 0 = the kernel writes nothing, bit 1 = reads nothing
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
-                                   int* status, const double* rho, double* jpart, cudaStream_t st);
+                                   int* status, const double* rho, double* jpart, int dbg, cudaStream_t st);
 // jpart (may be null): [chunk of 32 q, counted from q0][npair] partials of Eq. 4; J_p = their sum in order
 cudaError_t launch_jk_j_reduce(const double* jpart, int nchunks, int64_t npair, double* Jp, cudaStream_t st);
 // X[(q, i)][a_pad] -> planes6[t][i][qcol[q] + a] (pitch6), e6[g][i] from xmax; qgroup[q] = group of q,

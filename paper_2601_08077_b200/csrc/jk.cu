@@ -508,9 +508,6 @@ __global__ void __launch_bounds__(256) jk_j_unpack_kernel(const double* __restri
 }
 
 // ---------------------------------------------------------------------------
-static int g_jk_dbg = 0;
-void set_jk_debug_flags(int flags) { g_jk_dbg = flags; }
-
 static unsigned tile_pairs(int nao) {
   const unsigned T = (unsigned)((nao + 31) / 32);
   return T * (T + 1) / 2;
@@ -565,26 +562,26 @@ template <int S>
 static cudaError_t unpack_split_s(dim3 grid, int smem, cudaStream_t st, const double* Bp, int nao, int naux, int q0,
                                   int q1, const uint32_t* emax, int32_t* e5, int8_t* planes5, int64_t pitch,
                                   int64_t plane_stride, int* status, const double* rho, double* jpart,
-                                  long long npair) {
+                                  long long npair, int dbg) {
   // set on every launch (s >= 6 stages more than 48 KB): the attribute is per device
   cudaError_t err = cudaFuncSetAttribute(jk_unpack_split_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          2 * S * 32 * kUnpackPitch);
   if (err != cudaSuccess) return err;
   jk_unpack_split_kernel<S><<<grid, 256, smem, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5, pitch, plane_stride,
-                                                     status, g_jk_dbg, rho, jpart, npair);
+                                                     status, dbg, rho, jpart, npair);
   return cudaSuccess;
 }
 
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
-                                   int* status, const double* rho, double* jpart, cudaStream_t st) {
+                                   int* status, const double* rho, double* jpart, int dbg, cudaStream_t st) {
   const unsigned T128 = (unsigned)((nao + 127) / 128);
   if (pitch % 128 != 0 || pitch < 128 * (int64_t)T128) return cudaErrorInvalidValue;
   dim3 grid((unsigned)(2 * (128 / kUnpackRows)) * (T128 * (T128 + 1) / 2), (unsigned)((q1 - q0 + 31) / 32));
   const int smem = 2 * s * 32 * kUnpackPitch;
   cudaError_t err = cudaSuccess;
   DFE_DISPATCH_S(s, (err = unpack_split_s<SS>(grid, smem, st, Bp, nao, naux, q0, q1, emax, e5, planes5, pitch,
-                                              plane_stride, status, rho, jpart, (long long)nao * (nao + 1) / 2)));
+                                              plane_stride, status, rho, jpart, (long long)nao * (nao + 1) / 2, dbg)));
   if (err != cudaSuccess) return err;
   count_launch();
   return cudaGetLastError();

@@ -680,3 +680,63 @@ def test_jk_alternative_gemm5_paths(dfe, gpu_ws, flags):
             assert O.rel_frobenius(K, K_emu) <= 1e-14
     finally:
         dfe.lib.df_debug_set_gemm_flags(0)
+
+
+def test_two_contexts_two_streams_concurrent(dfe, gpu_ws):
+    """one workspace per concurrent stream.  Two contexts, each with its own
+    workspace, run different builds (and a GEMM) on two streams at the same time, several rounds
+    interleaved; every result equals the serial one of the default context bit for bit.  The policy
+    mode and the debug knobs belong to the context."""
+    nao, nocc = 150, 20
+    cases = []
+    for seed, naux, s in ((61, 1100, 4), (62, 700, 6)):
+        Bp = G.make_B_packed(nao, naux, seed=seed)
+        Cocc = G.make_C_occ(nao, nocc, seed=seed)
+        D = G.make_density(Cocc)
+        Bd, Cd, Dd = dev(Bp), dev(Cocc), dev(D)
+        J = torch.empty((nao, nao), dtype=torch.float64, device=DEV)
+        K = torch.empty_like(J)
+        dfe.df_jk_build_slices(Bd, nao, naux, Cd, nocc, Dd, s, J, K)
+        cases.append((Bd, naux, Cd, Dd, s, J, K))
+    A, B = G.make_gemm_inputs(300, 260, 1500, seed=63)
+    Ad, Bgd = dev(A), dev(B)
+    Cser = torch.empty((300, 260), dtype=torch.float64, device=DEV)
+    dfe.df_emul_gemm(Ad, Bgd, Cser, 300, 260, 1500, 1e-8)
+    torch.cuda.synchronize()
+    nbytes = max(dfe.df_jk_workspace_bytes_blocks(nao, 1100, nocc, 6, 3), dfe.df_emul_gemm_workspace_bytes(300, 260, 1500, 8))
+    ctxs = [dfe.Context(nbytes), dfe.Context(nbytes)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    try:
+        outs = []
+        for rnd in range(4):
+            for i in (0, 1):
+                Bd, naux, Cd, Dd, s, _, _ = cases[(i + rnd) % 2]
+                J2 = torch.full((nao, nao), np.nan, dtype=torch.float64, device=DEV)
+                K2 = torch.full_like(J2, np.nan)
+                C2 = torch.full_like(Cser, np.nan)
+                with torch.cuda.stream(streams[i]):
+                    ctxs[i].jk_build_slices(Bd, nao, naux, Cd, nocc, Dd, s, J2, K2)
+                    ctxs[i].emul_gemm(Ad, Bgd, C2, 300, 260, 1500, 1e-8)
+                outs.append(((i + rnd) % 2, J2, K2, C2))
+        torch.cuda.synchronize()
+        for which, J2, K2, C2 in outs:
+            assert torch.equal(J2, cases[which][5]) and torch.equal(K2, cases[which][6])
+            assert torch.equal(C2, Cser)
+        assert ctxs[0].last_status() == 0 and ctxs[1].last_status() == 0
+        # per-context policy: nominal mode takes one slice less at this tolerance, guarded is unchanged
+        ctxs[0].set_policy_mode(dfe.DF_MODE_NOMINAL)
+        Cn, Cg = torch.empty_like(Cser), torch.empty_like(Cser)
+        ctxs[0].emul_gemm(Ad, Bgd, Cn, 300, 260, 1500, 1e-8)
+        ctxs[1].emul_gemm(Ad, Bgd, Cg, 300, 260, 1500, 1e-8)
+        torch.cuda.synchronize()
+        assert dfe.df_slices_for_tol(1e-8, dfe.DF_MODE_NOMINAL) < dfe.df_slices_for_tol(1e-8)
+        assert np.array_equal(Cn.cpu().numpy(), O.emul_gemm(A, B, dfe.df_slices_for_tol(1e-8, dfe.DF_MODE_NOMINAL)))
+        assert torch.equal(Cg, Cser)
+        # per-context debug knobs: an alternative code path on one context only, same bits
+        ctxs[1].set_debug_flags((1 << 20) | 8)
+        ctxs[1].emul_gemm(Ad, Bgd, Cg, 300, 260, 1500, 1e-8)
+        torch.cuda.synchronize()
+        assert torch.equal(Cg, Cser)
+    finally:
+        for c in ctxs:
+            c.close()

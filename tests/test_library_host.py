@@ -186,3 +186,22 @@ def test_caller_schedule_matches_table1_and_oracle():
     # a noisy sequence never lowers the precision again
     lv = [l for l, _ in policy.schedule([1e-3, 1e-9, 1e-3, 1e-12, 1e-5, 1e-15, 1.0])]
     assert lv == [4, 4, 2, 2, 1, 1, 0, 0]  # 1e-9 < 5e-9 -> level 2; 1e-12 -> level 1
+
+
+def test_context_entry_points_fail_loudly_without_a_device(dfe):
+    """No GPU here: creating a context reports DF_ERR_DEVICE, a NULL context DF_ERR_NULL -- nothing
+    falls back to the CPU."""
+    import ctypes as C
+
+    try:
+        import torch
+
+        if torch.cuda.is_available():
+            pytest.skip("a CUDA device is present")
+    except ImportError:
+        pass
+    h = C.c_void_p()
+    assert dfe.lib.df_context_create(C.c_void_p(256), 1 << 20, C.byref(h)) == -5
+    assert dfe.lib.df_context_create(None, 1 << 20, C.byref(h)) == -1
+    assert dfe.lib.df_context_jk_build(None, None, 1, 1, None, 1, None, 1e-6, None, None, None) == -1
+    assert dfe.lib.df_context_destroy(None) == -1
