@@ -235,7 +235,7 @@ def run_ours(args, cfg):
     nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc
     # ---- inputs (synthetic, seeded).  With N ranks every rank owns one
     # q-shard of `naux` auxiliary functions of an N*naux basis (weak scaling).
-    B = G.make_B_packed_torch(nao, naux, cfg.seed + rank, device=dev)
+    B = G.make_B_packed_torch(nao, naux, cfg.seed + rank, device=dev, decay=args.screen)
     C0 = G.make_C_occ(nao, nocc, cfg.seed)
     D0 = G.make_density(C0)
     if args.config == "largest":
@@ -328,7 +328,28 @@ def run_ours(args, cfg):
     assert bool(torch.equal(K, K.T)) and bool(torch.equal(J, J.T))
 
     # ---- the same steps with per-kernel-class timing (roofline numerators)
+    p.df_screen_stats()
     ms_prof, prof = profiled(args.steps, args.warmup)
+    scr_active, scr_total = p.df_screen_stats()
+    screening = {"decay": args.screen, "active_k_blocks": scr_active, "all_k_blocks": scr_total,
+                 "n_scr_over_nbf2": scr_active / max(1, scr_total),
+                 "what": "(256 rows (q, i), 128 columns j) blocks of GEMM(5)'s left operand that hold a non-zero "
+                         "digit at the step's slice count; the others are neither written, loaded nor multiplied "
+                         "(PAPER.md:120, 164; exact: J, K are the dense results)"}
+    if args.screen > 0.0:
+        # the same data and steps with the screening switched off (every block written and multiplied)
+        p.df_debug_set_gemm_flags(1 << 25)
+        for i in range(args.warmup):
+            step(i, True)
+        ms_dense = timed(args.steps, True, args.warmup)
+        K_dense = K.clone()
+        _, prof_dense = profiled(args.steps, args.warmup)
+        p.df_debug_set_gemm_flags(0)
+        step(args.warmup + args.steps - 1, True)
+        torch.cuda.synchronize()
+        screening.update({"ms_per_step_screening_off": ms_dense / args.steps,
+                          "kernel_ms_per_step_screening_off": {k: v[0] / args.steps for k, v in prof_dense.items() if v[1]},
+                          "bit_identical_to_screening_off": bool(torch.equal(K, K_dense))})
 
     # ---- end to end through the C-ABI with HOST buffers: D_k, C_k from pinned memory in, J, K
     # out, every step; B stays resident (it is constant over the SCF).
@@ -412,6 +433,7 @@ def run_ours(args, cfg):
         "config": {"workload": workload_name(args.config, cfg) + (", 12-step adaptive SCF sequence" if nseq == NSEQ else ", tol alternating 1e-6 / 1e-10") + ", one q-shard per GPU",
                    "slices_per_step": used, "tol_per_step": [tols[i % nseq] for i in range(args.warmup, args.warmup + args.steps)],
                    "l2": "inputs larger than L2: packed B is %.1f GB and every step streams it" % (B.numel() * 8 / 1e9),
+                   "screen_decay": args.screen,
                    "workspace_gb": ws.view.numel() / 1e9, "q_blocks_per_launch": nblk},
         "effective_fp64_tflops": flops_per_build(cfg) * value / 1e12,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -441,6 +463,7 @@ def run_ours(args, cfg):
                          "traffic_source": NCU_TABLE if table else None},
         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items() if v[1]},
         "profiled_ms_per_step": ms_prof / args.steps,
+        "screening": screening,
     }
     if args.config == "largest":
         # configs[4]: "a single K build reported separately": everything but rho and J (pass A, the
@@ -629,6 +652,8 @@ def main():
     ap.add_argument("--ref-q", dest="ref_q", type=int, default=128)
     ap.add_argument("--cpu-q", dest="cpu_q", type=int, default=512)
     ap.add_argument("--sizes", type=int, nargs="+", default=[1024, 2048, 4096, 8192, 16384])
+    ap.add_argument("--screen", type=float, default=0.0,
+                    help="decay of a Schwarz-like fall-off exp(-decay |i - j|) of B (0: the configs' unstructured B)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-level0", dest="level0", action="store_false")
     args = ap.parse_args()

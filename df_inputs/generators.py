@@ -5,6 +5,8 @@ Recipes (stated again in DESIGN.md "Input recipe"):
 * B^q_ij, packed lower-triangular, shape (npair, naux), q fastest,
   p(i, j) = i(i+1)/2 + j for i >= j.  Entries = sign * 10^u, u ~ U(-8, 0) real,
   times a per-q decay exp(-q / naux)                      (configs 0, 2, 3, 4).
+* Screened variant: the same entries times exp(-decay |i - j|) (a Schwarz-like fall-off away from
+  the diagonal)                               (screening tests, bench --screen).
 * C_occ = first nocc columns of the Q factor of a Gaussian nao x nao matrix,
   D = 2 C_occ C_occ^T                                      (configs 0, 2, 3, 4).
 * GEMM sweep: entries sign * 2^e, e ~ U(-30, 0) REAL, plus an
@@ -65,6 +67,18 @@ def make_B_packed(nao: int, naux: int, seed: int, dtype=np.float64) -> np.ndarra
     return np.ascontiguousarray(B, dtype=dtype)
 
 
+def make_B_packed_screened(nao: int, naux: int, seed: int, decay: float = 0.25) -> np.ndarray:
+    """Packed B with a Schwarz-like decay away from the diagonal: the entries of make_B_packed times
+    exp(-decay |i - j|), the shape a screened three-index tensor of a spatially extended molecule
+    has (the significant pairs number N_scr <= N_bf^2, normally O(N_bf)).  Far from the
+    diagonal the values fall below every slice of their row's scale, so whole blocks of digits are
+    zero."""
+    B = make_B_packed(nao, naux, seed)
+    il, jl = np.tril_indices(nao)
+    B *= np.exp(-decay * (il - jl))[:, None]
+    return np.ascontiguousarray(B)
+
+
 def make_C_occ(nao: int, nocc: int, seed: int) -> np.ndarray:
     rng = np.random.default_rng(seed + 1000003)
     G = rng.standard_normal((nao, nao))
@@ -122,11 +136,13 @@ def make_scf_sequence(D_star: np.ndarray, nocc: int, nsteps: int, seed: int):
     return out
 
 
-def make_B_packed_torch(nao: int, naux: int, seed: int, device="cuda", chunk_pairs: int = 1 << 16):
+def make_B_packed_torch(nao: int, naux: int, seed: int, device="cuda", chunk_pairs: int = 1 << 16,
+                        decay: float = 0.0):
     """Device-side generation of packed B for the configs too large for host
     RAM/time (configs 3, 4).  Same distribution as make_B_packed; NOT the same
     bytes (a different generator) -- the oracle always reads these bytes back,
-    it never regenerates them."""
+    it never regenerates them.  decay > 0: the screened variant, entries
+    times exp(-decay |i - j|) (make_B_packed_screened)."""
     import torch
 
     n = npair(nao)
@@ -142,6 +158,13 @@ def make_B_packed_torch(nao: int, naux: int, seed: int, device="cuda", chunk_pai
         blk = torch.exp(u.mul_(8.0 * ln10).sub_(8.0 * ln10))
         blk.mul_(decay[None, :])
         blk = torch.where(sgn < 0.5, -blk, blk)
+        if decay > 0.0:
+            pidx = torch.arange(p0, p1, dtype=torch.float64, device=device)
+            i = torch.floor((torch.sqrt(8.0 * pidx + 1.0) - 1.0) * 0.5)
+            i = torch.where(i * (i + 1) / 2 > pidx, i - 1, i)
+            i = torch.where((i + 1) * (i + 2) / 2 <= pidx, i + 1, i)
+            j = pidx - i * (i + 1) / 2
+            blk.mul_(torch.exp(-decay * (i - j))[:, None])
         B[p0:p1].copy_(blk)
         del u, sgn, blk
     return B

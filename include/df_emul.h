@@ -125,6 +125,7 @@ int df_context_jk_build_planned_slices(df_context* ctx, const void* plan, int sm
                                        int64_t nao, int64_t naux, const double* C_occ, int64_t nocc,
                                        const double* D, int s, double* J, double* K, void* stream);
 int df_context_last_status(df_context* ctx, void* stream, int* status);
+int df_context_screen_stats(df_context* ctx, void* stream, int64_t* active, int64_t* total);
 
 /* ---- the two mandated entry points (default context) --------------------- */
 
@@ -154,10 +155,12 @@ int df_jk_build(const double* B_packed, int64_t nao, int64_t naux,
  * prefix property (R3: a build with s slices reads the first s of smax
  * planes).  A plan is a caller-owned device buffer (256-byte aligned) of
  * df_jk_plan_bytes() bytes holding them: naux x nao x (8 + round_up(nao,128) x smax)
- * bytes, 37 GB at config 3 with smax = 6.  df_jk_plan_create() fills it (row maxima
- * + unpack + split of all q, the H2 row of SURVEY.md section 8(a)); it needs a
- * registered workspace only for the status word.  DF_ERR_WORKSPACE if plan_bytes is
- * too small. */
+ * bytes plus the tile maxima of the screening mask (4 bytes per 32 x 32 tile pair and q),
+ * 37 GB at config 3 with smax = 6.  df_jk_plan_create() fills it (row maxima
+ * + unpack + split of all q, the H2 row of SURVEY.md section 8(a)); of the registered
+ * workspace it uses the status words and, when it is large enough (4 bytes per 256 rows
+ * (q, i) and 32 K blocks behind the first 256 bytes), room for the screening mask at smax
+ * slices.  DF_ERR_WORKSPACE if plan_bytes is too small. */
 int64_t df_jk_plan_bytes(int64_t nao, int64_t naux, int smax);
 int df_jk_plan_create(const double* B_packed, int64_t nao, int64_t naux, int smax,
                       void* plan, int64_t plan_bytes, void* stream);
@@ -188,6 +191,16 @@ int df_jk_build_slices(const double* B_packed, int64_t nao, int64_t naux,
 /* Copies the device status word (OR of DF_STATUS_* bits since the last call of
  * this function) to *status (host) and clears it.  SYNCHRONISES `stream`. */
 int df_last_status(void* stream, int* status);
+
+/* Screening ("N_scr <= N_bf^2", PAPER.md:164 grouped GEMM).
+ * Every J/K build judges, from the row scales and the maxima of 32 x 32 tiles its first pass over B
+ * leaves, which (256 rows (q, i), 128 columns j) blocks of GEMM(5)'s left operand hold no non-zero digit
+ * at the build's slice count (every |B^q_ij| below 2^(e_qi - 8 s - 1)); those blocks are neither written by
+ * the unpack pass nor loaded or multiplied by GEMM(5).  Only exact zeros are skipped: J and K are the
+ * dense results bit for bit.  *active / *total (host) receive the number of active and of all such
+ * blocks summed over the builds (and plan creations) since the last call; the counters are cleared.
+ * SYNCHRONISES `stream`.  N_scr / N_bf^2 of the paper's FLOP model ~ active / total. */
+int df_screen_stats(void* stream, int64_t* active, int64_t* total);
 
 /* ---- debug exports (tests only; not on the timed path) ------------------ */
 
@@ -236,7 +249,8 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
  *   bit 20     no cta_group::2 pair tiles                            walked (2 bits), swizzle (2 bits)
  *   bit 22     GEMM(5) N halves on multicast CTA pairs, never on MMA pairs
  *   bit 23     GEMM epilogue moves FP64 through the staged 16-byte path, never 256-bit accesses
- *   bit 24     df_emul_gemm keeps 128-column tiles at s <= 3 (default: 256 columns at s <= 2, 160 at s = 3) */
+ *   bit 24     df_emul_gemm keeps 128-column tiles at s <= 3 (default: 256 columns at s <= 2, 160 at s = 3)
+ *   bit 25     no screening: every K block of GEMM(5) is written, loaded and multiplied */
 int df_debug_set_gemm_flags(int flags);
 
 /* Number of GPU kernels this library has launched in this process. */

@@ -13,7 +13,7 @@ _EXPORTS = (
     "DF_MODE_NOMINAL", "DF_MODE_GUARDED", "DF_STATUS_NONFINITE", "DF_STATUS_RANGE",
     "df_slices_for_tol", "df_num_int8_gemms", "df_kflush", "df_set_policy_mode", "df_plane_pitch",
     "df_emul_gemm_workspace_bytes", "df_jk_workspace_bytes", "df_jk_workspace_bytes_blocks", "df_set_workspace",
-    "df_emul_gemm", "df_emul_gemm_slices", "df_jk_build", "df_jk_build_slices", "df_last_status",
+    "df_emul_gemm", "df_emul_gemm_slices", "df_jk_build", "df_jk_build_slices", "df_last_status", "df_screen_stats",
     "df_jk_plan_bytes", "df_jk_planned_workspace_bytes", "df_jk_build_planned", "df_jk_build_planned_slices",
     "df_debug_split_rows", "df_debug_split_cols", "df_debug_weight_sums", "df_debug_jk_build",
     "df_debug_set_gemm_flags", "df_launch_count", "df_profile_enable", "df_profile_read", "df_debug_mma_peak",

@@ -68,6 +68,8 @@ _SIG = {
     "df_context_jk_build_planned": (_i32, [_vp, _vp, _i32, _vp, _i64, _i64, _vp, _i64, _vp, _f64, _vp, _vp, _vp]),
     "df_context_jk_build_planned_slices": (_i32, [_vp, _vp, _i32, _vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
     "df_context_last_status": (_i32, [_vp, _vp, C.POINTER(C.c_int)]),
+    "df_context_screen_stats": (_i32, [_vp, _vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
+    "df_screen_stats": (_i32, [_vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
     "df_debug_split_rows": (_i32, [_vp, _i64, _i64, _i32, _vp, _vp, _vp]),
     "df_debug_split_cols": (_i32, [_vp, _i64, _i64, _i32, _vp, _vp, _vp]),
     "df_debug_weight_sums": (_i32, [_vp, _vp, _i64, _i64, _i64, _i32, _i32, _i32, _vp, _vp]),
@@ -253,6 +255,12 @@ class Context:
         _check(lib.df_context_last_status(self.handle, _stream(stream), C.byref(out)), "df_context_last_status")
         return int(out.value)
 
+    def screen_stats(self, stream=None):
+        a, t = C.c_int64(0), C.c_int64(0)
+        _check(lib.df_context_screen_stats(self.handle, _stream(stream), C.byref(a), C.byref(t)),
+               "df_context_screen_stats")
+        return int(a.value), int(t.value)
+
 
 # ---- the two entry points -----------------------------------------------------------------
 def df_emul_gemm(A, B, Cout, m, n, k, tol, stream=None) -> None:
@@ -334,6 +342,13 @@ def df_last_status(stream=None) -> int:
     out = C.c_int(0)
     _check(lib.df_last_status(_stream(stream), C.byref(out)), "df_last_status")
     return int(out.value)
+
+
+def df_screen_stats(stream=None):
+    """(active, total) K blocks of GEMM(5)'s left operand since the last call; synchronises."""
+    a, t = C.c_int64(0), C.c_int64(0)
+    _check(lib.df_screen_stats(_stream(stream), C.byref(a), C.byref(t)), "df_screen_stats")
+    return int(a.value), int(t.value)
 
 
 # ---- debug exports ------------------------------------------------------------------------

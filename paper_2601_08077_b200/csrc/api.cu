@@ -33,6 +33,7 @@ struct df_context {
   bool wide_n() const { return !((env.flags >> 24) & 1); }        // bit 24: df_emul_gemm never takes wide tiles
   bool g5_pair_halves() const { return !((env.flags >> 22) & 1); }  // bit 22: N halves never on MMA pairs
   int jk_dbg() const { return (env.flags >> 4) & 3; }             // bits 4, 5: unpack kernel without stores / loads
+  bool screening() const { return !((env.flags >> 25) & 1); }     // bit 25: no screening of zero K blocks
 };
 
 namespace dfe {
@@ -235,6 +236,8 @@ struct JkWs {
   int* status;
   double *rho, *rho_part;
   uint32_t* emax5;
+  uint32_t* tilemax;  // [32 x 32 tile pair][naux]: the tile maxima pass A leaves for the screening mask
+  uint32_t* kmask;    // [256-row block of the super-block][mask words]: active K blocks of GEMM(5)
   double* Jp;
   double* jpart;  // [ceil(naux / 32)][npair] chunk partials of Eq. 4 (plain builds)
   uint32_t* cmaxC;
@@ -254,18 +257,19 @@ struct JkWs {
 };
 
 // Plan buffer (df_jk_plan_create): everything about B that does not change over an SCF.
-//   [emax5: nao x naux u32][e5: (q, i) i32][planes: smax x (q, i) x pitch int8]
+//   [emax5: nao x naux u32][tilemax: tile pairs x naux u32][e5: (q, i) i32][planes: smax x (q, i) x pitch int8]
 // The digit planes have the prefix property (R3): a build with s <= smax slices reads
 // the first s planes.
 struct PlanLayout {
-  int64_t pitch, rows, emax_off, e5_off, planes_off, plane_stride, bytes;
+  int64_t pitch, rows, emax_off, tilemax_off, e5_off, planes_off, plane_stride, bytes;
 };
 static PlanLayout plan_layout(int64_t nao, int64_t naux, int smax) {
   PlanLayout L;
   L.pitch = round_up(nao, 128);
   L.rows = naux * nao;
   L.emax_off = 0;
-  L.e5_off = round_up(L.rows * 4, 256);
+  L.tilemax_off = round_up(L.rows * 4, 256);
+  L.e5_off = L.tilemax_off + round_up(jk_rho_part_rows((int)nao) * naux * 4, 256);
   L.planes_off = L.e5_off + round_up(L.rows * 4, 256);
   L.plane_stride = L.rows * L.pitch;
   L.bytes = L.planes_off + smax * L.plane_stride;
@@ -288,6 +292,8 @@ static JkWs carve_jk(void* base, int64_t nao, int64_t naux, int64_t nocc, int s,
   w.rho = c.take<double>(naux);
   w.rho_part = c.take<double>(jk_rho_part_rows((int)nao) * naux);
   w.emax5 = planned ? nullptr : c.take<uint32_t>(nao * naux);
+  w.tilemax = planned ? nullptr : c.take<uint32_t>(jk_rho_part_rows((int)nao) * naux);
+  w.kmask = c.take<uint32_t>(((QS * nao + 255) / 256) * screen_mask_words(nao));
   w.Jp = c.take<double>(nao * (nao + 1) / 2);
   w.jpart = planned ? nullptr : c.take<double>(((naux + 31) / 32) * (nao * (nao + 1) / 2));
   w.cmaxC = c.take<uint32_t>(w.a_pad);
@@ -357,7 +363,8 @@ static int jk_impl(df_context& c, const double* Bp, int64_t nao, int64_t naux, c
   if (!planned) DFE_CK(cudaMemsetAsync(w.emax5, 0, sizeof(uint32_t) * nao * naux, st));
   {
     ProfScope ps(kPPassA, st);
-    DFE_CK(launch_jk_pass_a(Bp, (int)nao, (int)naux, D, w.rho_part, w.rho, w.emax5, st));
+    DFE_CK(launch_jk_pass_a(Bp, (int)nao, (int)naux, D, w.rho_part, w.rho, w.emax5,
+                            c.screening() ? w.tilemax : nullptr, st));
   }
   if (planned) {
     ProfScope ps(kPJGemv, st);
@@ -390,12 +397,23 @@ static int jk_impl(df_context& c, const double* Bp, int64_t nao, int64_t naux, c
     DFE_CK(cudaGetLastError());
     DFE_CK(cudaMemsetAsync(w.xmax, 0, sizeof(uint32_t) * ng * nao, st));
 
+    // screening: the K blocks of GEMM(5)'s left operand that hold a
+    // non-zero digit at s slices; the unpack pass writes and GEMM(5) reads only those
+    const uint32_t* kmask = nullptr;
+    if (c.screening()) {
+      const uint32_t* em = planned ? reinterpret_cast<const uint32_t*>(plan_b + PL.emax_off) : w.emax5;
+      const uint32_t* tmx = planned ? reinterpret_cast<const uint32_t*>(plan_b + PL.tilemax_off) : w.tilemax;
+      DFE_CK(launch_jk_screen_mask(em, tmx, (int)nao, (int)naux, (int)qs0, nq, s, w.kmask,
+                                   reinterpret_cast<unsigned long long*>(w.status + 8), st));
+      kmask = w.kmask;
+    }
+
     // H2: unpack + split packed B -> planes5 rows (q, i), contraction j (a plan holds them already)
     if (!planned) {
       ProfScope ps(kPUnpack, st);
       DFE_CK(launch_jk_unpack_split(Bp, (int)nao, (int)naux, (int)qs0, (int)qs1, w.emax5, s, w.e5, w.p5,
                                     w.pitchj, (int64_t)nq * nao * w.pitchj, w.status, w.rho,
-                                    w.jpart + (qs0 / 32) * npair, c.jk_dbg(), st));
+                                    w.jpart + (qs0 / 32) * npair, c.jk_dbg(), kmask, screen_mask_words(nao), st));
     }
     if (!planned && qs1 == naux) {
       ProfScope ps(kPJGemv, st);
@@ -446,6 +464,8 @@ static int jk_impl(df_context& c, const double* Bp, int64_t nao, int64_t naux, c
     g5.ldx = w.a_pad;
     g5.qgroup = w.qgroup;
     g5.xmax = w.xmax;
+    g5.kmask = kmask;
+    g5.kmask_words = screen_mask_words(nao);
       {
       ProfScope ps(kPGemm5, st);
       DFE_CK(launch_gemm_i8(g5, c.env, st));
@@ -632,18 +652,36 @@ int df_context_jk_plan_create(df_context* ctx, const double* B_packed, int64_t n
   cudaStream_t st = (cudaStream_t)stream;
   char* pb = static_cast<char*>(plan);
   uint32_t* emax = reinterpret_cast<uint32_t*>(pb + L.emax_off);
+  uint32_t* tilemax = reinterpret_cast<uint32_t*>(pb + L.tilemax_off);
   if (cudaMemsetAsync(emax, 0, sizeof(uint32_t) * L.rows, st) != cudaSuccess) return DF_ERR_CUDA;
   {
     ProfScope ps(kPPassA, st);
-    if (launch_jk_pass_a(B_packed, (int)nao, (int)naux, nullptr, nullptr, nullptr, emax, st) != cudaSuccess)
+    if (launch_jk_pass_a(B_packed, (int)nao, (int)naux, nullptr, nullptr, nullptr, emax, tilemax, st) != cudaSuccess)
       return DF_ERR_CUDA;
+  }
+  // the planes are written for the K blocks that are active at smax slices: every build with s <= smax
+  // reads a subset of them (its threshold 2^(e - 8 s - 1) is the larger one).  The mask of all q needs
+  // ceil(naux nao / 256) words per 32 K blocks of workspace behind the status words; without that room
+  // (or with screening off) every block is written.
+  const uint32_t* kmask = nullptr;
+  {
+    const int words = screen_mask_words(nao);
+    const int64_t need = 256 + round_up(((naux * nao + 255) / 256) * words * 4, 256);
+    if (ctx->screening() && ctx->ws_bytes >= need) {
+      uint32_t* km = reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + 256);
+      if (launch_jk_screen_mask(emax, tilemax, (int)nao, (int)naux, 0, (int)naux, smax, km,
+                                reinterpret_cast<unsigned long long*>(static_cast<int*>(ctx->ws) + 8), st) != cudaSuccess)
+        return DF_ERR_CUDA;
+      kmask = km;
+    }
   }
   {
     ProfScope ps(kPUnpack, st);
     if (launch_jk_unpack_split(B_packed, (int)nao, (int)naux, 0, (int)naux, emax, smax,
                                reinterpret_cast<int32_t*>(pb + L.e5_off),
                                reinterpret_cast<int8_t*>(pb + L.planes_off), L.pitch, L.plane_stride,
-                               (int*)ctx->ws, nullptr, nullptr, ctx->jk_dbg(), st) != cudaSuccess)
+                               (int*)ctx->ws, nullptr, nullptr, ctx->jk_dbg(), kmask, screen_mask_words(nao), st) !=
+        cudaSuccess)
       return DF_ERR_CUDA;
   }
   return DF_OK;
@@ -674,6 +712,20 @@ int df_context_last_status(df_context* ctx, void* stream, int* status) {
   if (cudaMemcpyAsync(status, ctx->ws, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return DF_ERR_CUDA;
   if (cudaMemsetAsync(ctx->ws, 0, sizeof(int), st) != cudaSuccess) return DF_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return DF_ERR_CUDA;
+  return DF_OK;
+}
+
+int df_context_screen_stats(df_context* ctx, void* stream, int64_t* active, int64_t* total) {
+  if (!ctx || !active || !total) return DF_ERR_NULL;
+  if (!ctx->ws) return DF_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  unsigned long long v[2] = {0ull, 0ull};
+  char* src = static_cast<char*>(ctx->ws) + 32;
+  if (cudaMemcpyAsync(v, src, sizeof(v), cudaMemcpyDeviceToHost, st) != cudaSuccess) return DF_ERR_CUDA;
+  if (cudaMemsetAsync(src, 0, sizeof(v), st) != cudaSuccess) return DF_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return DF_ERR_CUDA;
+  *active = (int64_t)v[0];
+  *total = (int64_t)v[1];
   return DF_OK;
 }
 
@@ -722,6 +774,10 @@ int df_jk_build_planned_slices(const void* plan, int smax, const double* B_packe
 }
 
 int df_last_status(void* stream, int* status) { return df_context_last_status(&g_default, stream, status); }
+
+int df_screen_stats(void* stream, int64_t* active, int64_t* total) {
+  return df_context_screen_stats(&g_default, stream, active, total);
+}
 
 // ---- debug exports (default context) --------------------------------------------------------
 

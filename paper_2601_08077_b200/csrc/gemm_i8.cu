@@ -61,6 +61,8 @@ struct GemmKernelParams {
   long long ldx;
   const int* qgroup;
   uint32_t* xmax;
+  const uint32_t* kmask;  // screening: active 128-column K blocks per 256-row block (null: all)
+  int kmask_words;
   int32_t* P;
   int dbg_chunk;
   // flattened slice-pair list: x = A plane offset>>4 within a stage, y = B plane offset>>4,
@@ -85,6 +87,34 @@ __device__ __forceinline__ void pass_weights(const GemmKernelParams& p, int ps, 
     slot0 = 2;
   }
 }
+
+// Screening (GEMM(5), internal.h GemmProblem::kmask): the K blocks of a tile that are loaded and
+// multiplied.  Bit J of the mask covers the contraction range [128 J, 128 J + 128), i.e. 128 / BK
+// consecutive K blocks.  Producer and MMA issuer walk the same sequence of active blocks.
+template <int BK>
+struct KBlocks {
+  uint32_t m[4];
+  __device__ __forceinline__ void load(const GemmKernelParams& p, int tm) {
+    if (p.kmask) {
+      const uint32_t* src = p.kmask + (long long)(tm >> 1) * p.kmask_words;
+#pragma unroll
+      for (int w = 0; w < 4; ++w) m[w] = w < p.kmask_words ? src[w] : 0u;
+    } else {
+#pragma unroll
+      for (int w = 0; w < 4; ++w) m[w] = 0xffffffffu;
+    }
+  }
+  __device__ __forceinline__ bool active(int kb) const {
+    const int J = (kb * BK) >> 7, wi = J >> 5;
+    const uint32_t w = wi == 0 ? m[0] : wi == 1 ? m[1] : wi == 2 ? m[2] : m[3];  // no dynamic register indexing
+    return (w >> (J & 31)) & 1u;
+  }
+  __device__ __forceinline__ int count(int nkb) const {
+    int n = 0;
+    for (int kb = 0; kb < nkb; ++kb) n += active(kb) ? 1 : 0;
+    return n;
+  }
+};
 
 // One unit of work of the persistent kernel: an output tile of one z item.
 struct WorkItem {
@@ -198,10 +228,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     if (lane == 0) {
       uint32_t it = 0;
       DFE_WORK_LOOP
+      KBlocks<BK> kbl;
+      kbl.load(p, tm);
       for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
         const int kc0 = zk0 + ch * p.kflush;
         const int kc1 = min(zk1, kc0 + p.kflush);
         const int nkb = (kc1 - kc0 + BK - 1) / BK;
+        const int nact = p.kmask ? kbl.count(nkb) : nkb;  // active K blocks (screening)
         for (int ps = 0; ps < npass; ++ps) {
           int w_hi, w_lo, slot0;
           pass_weights(p, ps, w_hi, w_lo, slot0);
@@ -210,24 +243,26 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
           // (K block j of plane t in plane slot j P + t): fewer, fuller stages -- the one-plane
           // pass of a two-pass tile was waiting 1230 cycles per K block for 4 MMAs
           const int kp = s / P;
-          const int nst = (nkb + kp - 1) / kp;
-          for (int sb = 0; sb < nst; ++sb, ++it) {
+          int kb = 0;
+          for (int left = nact; left > 0; ++it) {
             const uint32_t stage = it % S;
             const uint32_t ph = (it / S) & 1u;
+            const int nj = min(kp, left);  // K blocks in this stage
+            left -= nj;
             mbar_wait(&empty_bar[stage], ph ^ 1u);
             if (p.dbg_flags & 2) {
               if (CL != 4 || crank == 0) mbar_arrive(&full_bar[stage]);
               continue;
             }
             uint8_t* st = smem + (size_t)stage * p.stage_stride;
-            const int nj = min(kp, nkb - sb * kp);  // K blocks in this stage
             const uint32_t tx = (uint32_t)(nj * P) * (a_plane_bytes + b_plane_bytes);
             if (CL == 4) {
               // both CTAs' loads count on the LEADER's full barrier, which expects the bytes of both
               const uint32_t lead_bar = mapa_shared(smem_u32(&full_bar[stage]), 0u);
               if (crank == 0) mbar_expect_tx(&full_bar[stage], 2u * tx);
-              for (int j = 0; j < nj; ++j) {
-                const int kpos = kc0 + (sb * kp + j) * BK;
+              for (int j = 0; j < nj; ++j, ++kb) {
+                while (!kbl.active(kb)) ++kb;
+                const int kpos = kc0 + kb * BK;
                 for (int t = 0; t < P; ++t)
                   tma_load_3d_pair(st + (j * P + t) * a_plane_bytes, &p.mapA, lead_bar, kpos, tm * kTileM, t);
                 for (int u = 0; u < P; ++u)
@@ -237,8 +272,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
               continue;
             }
             mbar_expect_tx(&full_bar[stage], tx);
-            for (int j = 0; j < nj; ++j) {
-              const int kpos = kc0 + (sb * kp + j) * BK;
+            for (int j = 0; j < nj; ++j, ++kb) {
+              while (!kbl.active(kb)) ++kb;
+              const int kpos = kc0 + kb * BK;
               if (CL == 2) {
                 for (int t = 0; t < P; ++t)
                   tma_load_3d_mcast(st + (j * P + t) * a_plane_bytes + crank * (64 * BK), &p.mapA2, &full_bar[stage],
@@ -271,10 +307,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
     uint32_t it = 0, iter = 0;
     if (CL != 4 || crank == 0) {  // pair mode: only the leader CTA issues (and waits)
     DFE_WORK_LOOP
+    KBlocks<BK> kbl;
+    kbl.load(p, tm);
     for (int ch = chunk_lo; ch < chunk_hi; ++ch) {
       const int kc0 = zk0 + ch * p.kflush;
       const int kc1 = min(zk1, kc0 + p.kflush);
       const int nkb = (kc1 - kc0 + BK - 1) / BK;
+      const int nact = p.kmask ? kbl.count(nkb) : nkb;  // active K blocks (screening)
       for (int ps = 0; ps < npass; ++ps, ++iter) {
         const int pr0 = p.pass_start[ps], pr1 = p.pass_start[ps + 1];
         if (iter > 0) {
@@ -285,11 +324,14 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
         pass_weights(p, ps, w_hi_p, w_lo_p, slot0_p);
         const int P = min(s, w_hi_p - 1);
         const int kp = s / P;  // K blocks per stage (see the producer)
-        const int nst = (nkb + kp - 1) / kp;
         const uint32_t a_sub16 = (uint32_t)P * (a_plane_bytes >> 4), b_sub16 = (uint32_t)P * (b_plane_bytes >> 4);
-        for (int sb = 0; sb < nst; ++sb, ++it) {
+        int kb = 0;
+        uint32_t started = 0u;  // the accumulators of this pass hold a product already
+        for (int left = nact; left > 0; ++it) {
           const uint32_t stage = it % S;
           const uint32_t ph = (it / S) & 1u;
+          const int nj = min(kp, left);
+          left -= nj;
           mbar_wait(&full_bar[stage], ph);
           tc_fence_after();
           if (p.dbg_flags & 1) {
@@ -304,16 +346,21 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             continue;
           }
           const uint32_t lo_base = desc_lo0 | (smem_base16 + stage * stage16);
-          const int nj = min(kp, nkb - sb * kp);
+          // every lane walks the active blocks of this stage (kb stays warp-uniform); the elected lane issues
+          int kb_end = kb;
+          for (int j = 0; j < nj; ++j, ++kb_end)
+            while (!kbl.active(kb_end)) ++kb_end;
           if (elect_one()) {
-            for (int j = 0; j < nj; ++j) {
-              const int kb = sb * kp + j;
-              const int kpos = kc0 + kb * BK;
+            int kbe = kb;
+            for (int j = 0; j < nj; ++j, ++kbe) {
+              while (!kbl.active(kbe)) ++kbe;
+              const int kpos = kc0 + kbe * BK;
               const int nkk = (min(BK, kc1 - kpos) + 31) / 32;
               const uint32_t aj = (uint32_t)j * a_sub16, bj = (uint32_t)j * b_sub16;
               for (int kk = 0; kk < nkk; ++kk) {
                 const uint32_t lo = lo_base + 2u * kk;  // +32 bytes per K step, in 16-byte units
-                const uint32_t later = (kb | kk) ? 1u : 0u;
+                const uint32_t later = started;
+                started = 1u;
 #pragma unroll 4
                 for (int i = pr0; i < pr1; ++i) {
                   const uint4 e = p.pairs[i];
@@ -330,6 +377,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) gemm_i8_kernel(const __grid_c
             else if (CL == 2) mma_commit_mcast(&empty_bar[stage], (uint16_t)3);
             else mma_commit(&empty_bar[stage]);
           }
+          started = 1u;  // warp-uniform copies of the elected lane's state
+          kb = kb_end;
           __syncwarp();
         }
         if (elect_one()) {  // accumulators of this pass are complete (in both CTAs of a pair)
@@ -958,6 +1007,8 @@ cudaError_t launch_gemm_i8(const GemmProblem& g, const LaunchEnv& env, cudaStrea
   p.ldx = g.ldx;
   p.qgroup = g.qgroup;
   p.xmax = g.xmax;
+  p.kmask = g.mode == kEpiX ? g.kmask : nullptr;
+  p.kmask_words = g.kmask_words;
   p.P = g.P;
   p.dbg_chunk = g.dbg_chunk;
   p.dbg_flags = dbg_kernel;

@@ -115,6 +115,11 @@ struct GemmProblem {
   int64_t ldx;
   const int* qgroup;
   uint32_t* xmax;
+  // screening (kEpiX; may be null): kmask[(row / 256) * kmask_words + J / 32] bit J % 32 = the K block
+  // of columns 128 J .. 128 J + 127 of the 256-row block is active; inactive blocks are neither
+  // loaded nor multiplied (their planes need not exist)
+  const uint32_t* kmask;
+  int kmask_words;
   // kEpiInt32: P[(w - 2) * a_rows * b_rows + row * b_rows + col] of flush chunk `dbg_chunk`
   int32_t* P;
   int dbg_chunk;
@@ -130,16 +135,27 @@ cudaError_t launch_mma_peak(int n_mma, int iters, int grid, float* ms, cudaStrea
 // (atomicMax, must be zeroed).  rho == nullptr: the maxima alone (df_jk_plan_create); emax == nullptr:
 // rho alone, lower tiles only (planned builds).
 int64_t jk_rho_part_rows(int nao);
+// tilemax (may be null; only with emax): [jk_rho_part_rows(nao)][naux], upper word of the maximum of
+// every 32 x 32 tile pair and q (every element written) -- the input of the screening mask
 cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho_part, double* rho,
-                             uint32_t* emax, cudaStream_t st);
+                             uint32_t* emax, uint32_t* tilemax, cudaStream_t st);
+// screening mask of the 256-row blocks of the flattened rows (q - q0, i), q in [q0, q0 + nq):
+// mask[block][screen_mask_words(nao)], bit J = K block of columns 128 J .. may hold a non-zero digit at s
+// slices; stats[0] / stats[1] += active / all (block, K block) pairs
+inline int screen_mask_words(int64_t nao) { return (int)(((nao + 127) / 128 + 31) / 32); }
+cudaError_t launch_jk_screen_mask(const uint32_t* emax, const uint32_t* tilemax, int nao, int naux, int q0, int nq,
+                                  int s, uint32_t* mask, unsigned long long* stats, cudaStream_t st);
 // J_packed[p] = sum_q B[p, q] rho[q]
 cudaError_t launch_jk_j_gemv(const double* Bp, int64_t npair, int naux, const double* rho, double* Jp,
                              cudaStream_t st);
 // unpack + split q in [q0, q1): planes5[t][(q - q0) * nao + i][pitch], e5[(q - q0) * nao + i]
 // dbg (timing experiments): bit 0 = the kernel writes nothing, bit 1 = reads nothing
+// kmask (may be null): screening mask of [q0, q1); planes of inactive (256-row block, K block) pairs are
+// not written (and, where Eq. 4 does not ride on the block, not read)
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
-                                   int* status, const double* rho, double* jpart, int dbg, cudaStream_t st);
+                                   int* status, const double* rho, double* jpart, int dbg, const uint32_t* kmask,
+                                   int mask_words, cudaStream_t st);
 // jpart (may be null): [chunk of 32 q, counted from q0][npair] partials of Eq. 4; J_p = their sum in order
 cudaError_t launch_jk_j_reduce(const double* jpart, int nchunks, int64_t npair, double* Jp, cudaStream_t st);
 // X[(q, i)][a_pad] -> planes6[t][i][qcol[q] + a] (pitch6), e6[g][i] from xmax; qgroup[q] = group of q,

@@ -79,7 +79,8 @@ template <bool RHO, bool EMAX>
 __global__ void __launch_bounds__(256, EMAX ? 4 : 5) jk_pass_a_kernel(const double* __restrict__ Bp, int nao, int naux,
                                                         const double* __restrict__ D,
                                                         double* __restrict__ rho_part,
-                                                        uint32_t* __restrict__ emax) {
+                                                        uint32_t* __restrict__ emax,
+                                                        uint32_t* __restrict__ tilemax) {
   int TR, TC;
   bool lower;
   tile_of_block(blockIdx.y, 0, TR, TC, lower);
@@ -90,9 +91,11 @@ __global__ void __launch_bounds__(256, EMAX ? 4 : 5) jk_pass_a_kernel(const doub
   __shared__ double rho_sh[8][32];
   __shared__ double dw_sh[32][33];  // weighted density of this tile: (i == j ? 1 : 2) * 0.5 (D_ij + D_ji), 0 above the diagonal
   __shared__ uint32_t cmax_sh[32][32];  // [column of the tile][q]: max over the tile's rows
+  __shared__ uint32_t tmax_sh[32];      // [q]: max over the whole 32 x 32 tile (screening)
   if (EMAX && offdiag) {
     for (int idx = threadIdx.x; idx < 1024; idx += 256) cmax_sh[idx >> 5][idx & 31] = 0u;
   }
+  if (EMAX && threadIdx.x < 32) tmax_sh[threadIdx.x] = 0u;
   if (RHO) {
     for (int idx = threadIdx.x; idx < 1024; idx += 256) {
       const int rl = idx >> 5, cl = idx & 31;
@@ -156,11 +159,16 @@ __global__ void __launch_bounds__(256, EMAX ? 4 : 5) jk_pass_a_kernel(const doub
       if (R < nao) atomicMax(&emax[(long long)R * naux + q], hm[rr]);
     }
   }
+  if (EMAX && tilemax) atomicMax(&tmax_sh[lane], max(max(hm[0], hm[1]), max(hm[2], hm[3])));
   if (RHO) rho_sh[warp][lane] = rsum;
   if (RHO || (EMAX && offdiag)) __syncthreads();
   if (EMAX && offdiag && q_ok) {
     for (int cl = warp; cl < 32; cl += 8)  // TC < TR: every column of the tile is < nao
       atomicMax(&emax[(long long)(TC * 32 + cl) * naux + q], cmax_sh[cl][lane]);
+  }
+  if (EMAX && tilemax) {
+    if (!RHO && !offdiag) __syncthreads();  // the other variants have passed a barrier since the atomics
+    if (warp == 1 && q_ok) tilemax[(long long)blockIdx.y * naux + q] = tmax_sh[lane];
   }
   if (RHO) {
     if (warp == 0 && q_ok) {
@@ -331,7 +339,8 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
                                                               long long pitch, long long plane_stride,
                                                               int* __restrict__ status, int dbg,
                                                               const double* __restrict__ rho,
-                                                              double* __restrict__ jpart, long long npair) {
+                                                              double* __restrict__ jpart, long long npair,
+                                                              const uint32_t* __restrict__ kmask, int mask_words) {
   extern __shared__ __align__(16) uint8_t ubuf[];  // [2][S][32][kUnpackPitch]
   constexpr int kSubs = 128 / kUnpackRows;
   int A, B;
@@ -359,6 +368,14 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
   for (int r = 0; r < kUnpackRows; ++r) {
     const int R = A * 128 + (sub % kSubs) * kUnpackRows + r;
     if (R >= nao) break;  // block-uniform
+    // screening: bit B of the mask of the 256-row block of (q, R) -- lane = q in every warp, so the
+    // ballot is the same in all warps and the branches below are block-uniform
+    uint32_t act = 0xffffffffu;
+    if (kmask) {
+      const long long mb = ((long long)(q - q0) * nao + R) >> 8;
+      act = __ballot_sync(0xffffffffu, q_ok && ((kmask[mb * mask_words + (B >> 5)] >> (B & 31)) & 1u));
+      if (act == 0u && !do_j) continue;  // nothing to write, nothing to sum: the row is not even read
+    }
     const uint32_t hm = emax[(long long)R * naux + q];
     const int e = scale_index_from_hi(hm);
     if (lower && B == 0 && warp == 0 && q_ok) {
@@ -386,6 +403,7 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
       const int C = Cs + (lane >> 1);
       if ((lane & 1) == 0 && C <= R)  // C <= R < nao; a diagonal tile holds the rest as mirrors
         jp_chunk[(long long)R * (R + 1) / 2 + C] = k;
+      if (act == 0u) continue;  // Eq. 4 needs every element, the planes only the active blocks
     }
     uint32_t w[S][4];
 #pragma unroll
@@ -412,10 +430,65 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
     const long long row0 = ((long long)chunk * 32 * nao + R) * pitch + B * 128 + (lane & 7) * 16;
     for (int idx = warp * 4 + (lane >> 3); idx < S * 32; idx += 32) {
       const int t = idx >> 5, qq = idx & 31;
-      if (qq < nq_blk)
+      if (qq < nq_blk && ((act >> qq) & 1u))
         *reinterpret_cast<uint4*>(planes + t * plane_stride + row0 + (long long)qq * nao * pitch) =
             *reinterpret_cast<const uint4*>(buf + (t * 32 + qq) * kUnpackPitch + (lane & 7) * 16);
     }
+  }
+}
+
+// ---------------------------------------------------------------------------
+// Screening (PAPER.md:120 N_scr <= N_bf^2, "grouped
+// GEMM"): which 128-column K blocks of GEMM(5)'s left operand hold a non-zero digit at s slices.
+// An element of row (q, i) has its first s balanced digits all zero when |x| < 2^(e_qi - 8 s - 1)
+// (then |Q| <= 2^(62 - 8 s) < 0.498 * 2^(64 - 8 s), the largest magnitude whose top s digits vanish).
+// mask[mb] bit J = 0 says that in the 256 flattened rows (q, i) of block mb every element of columns
+// 128 J .. 128 J + 127 is below its row's threshold -- judged conservatively from the maxima of the
+// 32 x 32 tiles pass A left in tilemax.  The unpack pass writes no planes for such a block and GEMM(5)
+// neither loads it nor issues its MMAs: skipping exact zeros, the result is the dense one bit for bit.
+// A block with no active K block at all (zero rows) keeps bit 0, so its accumulators are written.
+// stats[0] / stats[1] += active / all (block, K block) pairs.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) jk_screen_mask_kernel(const uint32_t* __restrict__ emax,
+                                                             const uint32_t* __restrict__ tilemax, int nao, int naux,
+                                                             int q0, int nq, int s, int nJ, int words,
+                                                             uint32_t* __restrict__ mask,
+                                                             unsigned long long* __restrict__ stats) {
+  __shared__ uint32_t m_sh[4];
+  if (threadIdx.x < 4) m_sh[threadIdx.x] = 0u;
+  __syncthreads();
+  const long long row = (long long)blockIdx.x * 256 + threadIdx.x;
+  uint32_t m[4] = {0u, 0u, 0u, 0u};
+  if (row < (long long)nq * nao) {
+    const int ql = (int)(row / nao), i = (int)(row - (long long)ql * nao), q = q0 + ql;
+    const int e = scale_index_from_hi(__ldg(emax + (long long)i * naux + q));
+    const int eb = 1023 + e - 8 * s - 1;                       // biased exponent of the threshold
+    const uint32_t thr = eb > 0 ? (uint32_t)eb << 20 : 0u;      // below the normal range: everything counts
+    const unsigned ti = (unsigned)i >> 5;
+    const int T32 = (nao + 31) >> 5;
+    for (int tj = 0; tj < T32; ++tj) {
+      const unsigned hi = max(ti, (unsigned)tj), lo = min(ti, (unsigned)tj);
+      const uint32_t tm = __ldg(tilemax + (long long)(hi * (hi + 1) / 2 + lo) * naux + q);
+      if (tm >= thr && tm != 0u) m[tj >> 7] |= 1u << ((tj >> 2) & 31);
+    }
+  }
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    const uint32_t r = __reduce_or_sync(0xffffffffu, m[w]);
+    if ((threadIdx.x & 31) == 0 && r) atomicOr(&m_sh[w], r);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t any = 0u;
+    for (int w = 0; w < words; ++w) any |= m_sh[w];
+    if (!any) m_sh[0] = 1u;
+    int act = 0;
+    for (int w = 0; w < words; ++w) {
+      mask[(long long)blockIdx.x * words + w] = m_sh[w];
+      act += __popc(m_sh[w]);
+    }
+    atomicAdd(&stats[0], (unsigned long long)act);
+    atomicAdd(&stats[1], (unsigned long long)nJ);
   }
 }
 
@@ -516,14 +589,14 @@ static unsigned tile_pairs(int nao) {
 int64_t jk_rho_part_rows(int nao) { return tile_pairs(nao); }
 
 cudaError_t launch_jk_pass_a(const double* Bp, int nao, int naux, const double* D, double* rho_part, double* rho,
-                             uint32_t* emax, cudaStream_t st) {
+                             uint32_t* emax, uint32_t* tilemax, cudaStream_t st) {
   const unsigned qchunks = (unsigned)((naux + 31) / 32);
   if (emax && rho) {
-    jk_pass_a_kernel<true, true><<<dim3(qchunks, tile_pairs(nao)), 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax);
+    jk_pass_a_kernel<true, true><<<dim3(qchunks, tile_pairs(nao)), 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax, tilemax);
   } else if (rho) {
-    jk_pass_a_kernel<true, false><<<dim3(qchunks, tile_pairs(nao)), 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax);
+    jk_pass_a_kernel<true, false><<<dim3(qchunks, tile_pairs(nao)), 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax, nullptr);
   } else {
-    jk_pass_a_kernel<false, true><<<dim3(qchunks, tile_pairs(nao)), 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax);
+    jk_pass_a_kernel<false, true><<<dim3(qchunks, tile_pairs(nao)), 256, 0, st>>>(Bp, nao, naux, D, rho_part, emax, tilemax);
   }
   count_launch();
   if (rho) {
@@ -562,27 +635,39 @@ template <int S>
 static cudaError_t unpack_split_s(dim3 grid, int smem, cudaStream_t st, const double* Bp, int nao, int naux, int q0,
                                   int q1, const uint32_t* emax, int32_t* e5, int8_t* planes5, int64_t pitch,
                                   int64_t plane_stride, int* status, const double* rho, double* jpart,
-                                  long long npair, int dbg) {
+                                  long long npair, int dbg, const uint32_t* kmask, int mask_words) {
   // set on every launch (s >= 6 stages more than 48 KB): the attribute is per device
   cudaError_t err = cudaFuncSetAttribute(jk_unpack_split_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          2 * S * 32 * kUnpackPitch);
   if (err != cudaSuccess) return err;
   jk_unpack_split_kernel<S><<<grid, 256, smem, st>>>(Bp, nao, naux, q0, q1, emax, e5, planes5, pitch, plane_stride,
-                                                     status, dbg, rho, jpart, npair);
+                                                     status, dbg, rho, jpart, npair, kmask, mask_words);
   return cudaSuccess;
 }
 
 cudaError_t launch_jk_unpack_split(const double* Bp, int nao, int naux, int q0, int q1, const uint32_t* emax,
                                    int s, int32_t* e5, int8_t* planes5, int64_t pitch, int64_t plane_stride,
-                                   int* status, const double* rho, double* jpart, int dbg, cudaStream_t st) {
+                                   int* status, const double* rho, double* jpart, int dbg, const uint32_t* kmask,
+                                   int mask_words, cudaStream_t st) {
   const unsigned T128 = (unsigned)((nao + 127) / 128);
   if (pitch % 128 != 0 || pitch < 128 * (int64_t)T128) return cudaErrorInvalidValue;
   dim3 grid((unsigned)(2 * (128 / kUnpackRows)) * (T128 * (T128 + 1) / 2), (unsigned)((q1 - q0 + 31) / 32));
   const int smem = 2 * s * 32 * kUnpackPitch;
   cudaError_t err = cudaSuccess;
   DFE_DISPATCH_S(s, (err = unpack_split_s<SS>(grid, smem, st, Bp, nao, naux, q0, q1, emax, e5, planes5, pitch,
-                                              plane_stride, status, rho, jpart, (long long)nao * (nao + 1) / 2, dbg)));
+                                              plane_stride, status, rho, jpart, (long long)nao * (nao + 1) / 2, dbg, kmask,
+                                              mask_words)));
   if (err != cudaSuccess) return err;
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_jk_screen_mask(const uint32_t* emax, const uint32_t* tilemax, int nao, int naux, int q0, int nq,
+                                  int s, uint32_t* mask, unsigned long long* stats, cudaStream_t st) {
+  const int nJ = (nao + 127) / 128, words = (nJ + 31) / 32;
+  if (words > 4) return cudaErrorInvalidValue;
+  const long long nblk = ((long long)nq * nao + 255) / 256;
+  jk_screen_mask_kernel<<<(unsigned)nblk, 256, 0, st>>>(emax, tilemax, nao, naux, q0, nq, s, nJ, words, mask, stats);
   count_launch();
   return cudaGetLastError();
 }

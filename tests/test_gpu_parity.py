@@ -740,3 +740,60 @@ def test_two_contexts_two_streams_concurrent(dfe, gpu_ws):
     finally:
         for c in ctxs:
             c.close()
+
+
+@pytest.mark.parametrize("s", [3, 4, 6])
+def test_jk_screened_input_bit_exact(dfe, gpu_ws, s):
+    """on a B that decays away from the diagonal the
+    build skips the K blocks of GEMM(5)'s left operand whose digits all vanish at s slices.  Only exact
+    zeros are skipped, so X, the GEMM(6) scales and K are the DENSE oracle's, bit for bit; the counters
+    show that blocks were skipped; with screening off (bit 25) and through a plan the bits are the same."""
+    nao, naux, nocc = 600, 70, 40
+    Bp = G.make_B_packed_screened(nao, naux, seed=70 + s, decay=0.6)
+    Cocc = G.make_C_occ(nao, nocc, seed=70 + s)
+    D = G.make_density(Cocc)
+    dfe.df_screen_stats()
+    J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+    active, total = dfe.df_screen_stats()
+    nblk = (naux * nao + 255) // 256
+    assert total == nblk * 5 and 0 < active < 0.9 * total, (active, total)  # 5 K blocks of 128 columns
+    K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
+    J_ref, K_ref = O.df_jk_plain(Bp, nao, Cocc, D)
+    assert np.array_equal(X[:, :, :nocc], X_emu)
+    groups = O.q_groups(naux, nocc, s)
+    for g, (g0, g1) in enumerate(groups):
+        Xrow = np.transpose(X_emu[g0:g1], (1, 0, 2)).reshape(nao, -1)
+        assert np.array_equal(e6[g], O.scale_index(np.max(np.abs(Xrow), axis=1)))
+    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert O.rel_frobenius(J, J_ref) <= 1e-12
+    assert dfe.df_last_status() == 0
+    # screening off: every block is written, loaded and multiplied -- the same bits
+    dfe.lib.df_debug_set_gemm_flags(1 << 25)
+    try:
+        J0, K0, X0, _, _ = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+        assert dfe.df_screen_stats() == (0, 0)
+    finally:
+        dfe.lib.df_debug_set_gemm_flags(0)
+    assert np.array_equal(K0, K) and np.array_equal(X0, X) and np.array_equal(J0, J)
+    # a plan made at 6 slices holds every block a build with s <= 6 reads
+    Bd = dev(Bp)
+    plan = dfe.Plan(Bd, nao, naux, 6)
+    a6, t6 = dfe.df_screen_stats()
+    assert t6 == total and active <= a6 < total  # the mask at 6 slices covers the mask at s
+    J2 = torch.full((nao, nao), np.nan, dtype=torch.float64, device=DEV)
+    K2 = torch.full_like(J2, np.nan)
+    dfe.df_jk_build_planned_slices(plan, Bd, nao, naux, dev(Cocc), nocc, dev(D), s, J2, K2)
+    torch.cuda.synchronize()
+    assert np.array_equal(K2.cpu().numpy(), K) and np.array_equal(J2.cpu().numpy(), J)
+    assert dfe.df_screen_stats()[0] == active
+    plan.close()
+
+
+def test_jk_dense_input_keeps_every_block(dfe, gpu_ws):
+    """The configs' unstructured B: nothing is screened away."""
+    cfg = G.CONFIGS["tiny"]
+    Bp, Cocc, D = G.make_df_inputs(cfg)
+    dfe.df_screen_stats()
+    run_jk(dfe, Bp, cfg.nao, cfg.naux, Cocc, cfg.nocc, D, 4)
+    active, total = dfe.df_screen_stats()
+    assert active == total == (cfg.naux * cfg.nao + 255) // 256

@@ -103,11 +103,14 @@ def test_workspace_sizes(dfe):
 
 
 def test_plan_sizes(dfe):
-    """Plan = row maxima + scale indices (4 bytes each per (q, i)) + smax planes of (q, i) rows
-    padded to whole 128-byte lines; a planned build's workspace holds no GEMM(5) operand planes."""
+    """Plan = row maxima + scale indices (4 bytes each per (q, i)) + the maxima of the 32 x 32 tile
+    pairs (4 bytes per pair and q; the screening mask's input) + smax planes of (q, i) rows padded
+    to whole 128-byte lines; a planned build's workspace holds no GEMM(5) operand planes."""
     rows = 4000 * 1200
-    assert dfe.df_jk_plan_bytes(1200, 4000, 6) == 2 * rows * 4 + 6 * rows * 1280
-    assert dfe.df_jk_plan_bytes(100, 7, 1) == 2 * 2816 + 700 * 128
+    pairs32 = 38 * 39 // 2  # ceil(1200 / 32) tiles per side
+    r256 = lambda n: (n + 255) // 256 * 256  # every section starts on a 256-byte boundary
+    assert dfe.df_jk_plan_bytes(1200, 4000, 6) == 2 * rows * 4 + r256(pairs32 * 4000 * 4) + 6 * rows * 1280
+    assert dfe.df_jk_plan_bytes(100, 7, 1) == 2 * 2816 + 512 + 700 * 128  # 10 tile pairs x 7 q x 4 B -> 512
     w = dfe.df_jk_workspace_bytes_blocks(1200, 4000, 150, 4, 8)
     wp = dfe.df_jk_planned_workspace_bytes(1200, 4000, 150, 4, 8)
     assert 0 < wp <= w - 4 * rows * 1280
