@@ -235,7 +235,7 @@ def run_ours(args, cfg):
     nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc
     # ---- inputs (synthetic, seeded).  With N ranks every rank owns one
     # q-shard of `naux` auxiliary functions of an N*naux basis (weak scaling).
-    B = G.make_B_packed_torch(nao, naux, cfg.seed + rank, device=dev, decay=args.screen)
+    B = G.make_B_packed_torch(nao, naux, cfg.seed + rank, device=dev, offdiag_decay=args.screen)
     C0 = G.make_C_occ(nao, nocc, cfg.seed)
     D0 = G.make_density(C0)
     if args.config == "largest":

@@ -137,12 +137,12 @@ def make_scf_sequence(D_star: np.ndarray, nocc: int, nsteps: int, seed: int):
 
 
 def make_B_packed_torch(nao: int, naux: int, seed: int, device="cuda", chunk_pairs: int = 1 << 16,
-                        decay: float = 0.0):
+                        offdiag_decay: float = 0.0):
     """Device-side generation of packed B for the configs too large for host
     RAM/time (configs 3, 4).  Same distribution as make_B_packed; NOT the same
     bytes (a different generator) -- the oracle always reads these bytes back,
-    it never regenerates them.  decay > 0: the screened variant, entries
-    times exp(-decay |i - j|) (make_B_packed_screened)."""
+    it never regenerates them.  offdiag_decay > 0: the screened variant,
+    entries times exp(-offdiag_decay |i - j|) (make_B_packed_screened)."""
     import torch
 
     n = npair(nao)
@@ -158,13 +158,13 @@ def make_B_packed_torch(nao: int, naux: int, seed: int, device="cuda", chunk_pai
         blk = torch.exp(u.mul_(8.0 * ln10).sub_(8.0 * ln10))
         blk.mul_(decay[None, :])
         blk = torch.where(sgn < 0.5, -blk, blk)
-        if decay > 0.0:
+        if offdiag_decay > 0.0:
             pidx = torch.arange(p0, p1, dtype=torch.float64, device=device)
             i = torch.floor((torch.sqrt(8.0 * pidx + 1.0) - 1.0) * 0.5)
             i = torch.where(i * (i + 1) / 2 > pidx, i - 1, i)
             i = torch.where((i + 1) * (i + 2) / 2 <= pidx, i + 1, i)
             j = pidx - i * (i + 1) / 2
-            blk.mul_(torch.exp(-decay * (i - j))[:, None])
+            blk.mul_(torch.exp(-offdiag_decay * (i - j))[:, None])
         B[p0:p1].copy_(blk)
         del u, sgn, blk
     return B
