@@ -108,42 +108,46 @@ __global__ void col_scale_kernel(const uint32_t* __restrict__ cmax, long long n,
 // ---------------------------------------------------------------------------
 // Vectorised row split: ld % 4 == 0 and a 32-byte aligned base.  One block per row.
 // ---------------------------------------------------------------------------
-constexpr int kRowChunk = 1024;  // elements per block iteration: 256 threads x 4
-template <int S>
-__global__ void __launch_bounds__(256) split_rows_v4_kernel(const double* __restrict__ X, long long cols, long long ld,
-                                                            int32_t* __restrict__ e, int8_t* __restrict__ planes,
-                                                            long long pitch, long long plane_stride,
-                                                            int* __restrict__ status) {
+// NT threads per block (256, or 512 for long rows: more loads in flight per resident row).  The launcher
+// limits the resident blocks per SM (through the dynamic shared memory it asks for) so that the rows in
+// flight stay well inside L2 and the digit pass finds its row there: at 16384 columns eight blocks
+// per SM hold 151 MB of rows and the second pass read all of them from HBM again (ncu: 4.1 GB for 2.1).
+template <int S, int NT>
+__global__ void __launch_bounds__(NT) split_rows_v4_kernel(const double* __restrict__ X, long long cols, long long ld,
+                                                           int32_t* __restrict__ e, int8_t* __restrict__ planes,
+                                                           long long pitch, long long plane_stride,
+                                                           int* __restrict__ status) {
+  constexpr int kChunk = 4 * NT;  // elements per block iteration
   const long long row = blockIdx.x;
   const double* x = X + row * ld;
-  __shared__ uint32_t wmax[8];
+  __shared__ uint32_t wmax[NT / 32];
   __shared__ int e_sh;
-  __shared__ __align__(16) uint32_t stage[2][S][256];  // [buffer][plane][thread]: 4 digit bytes per thread
+  __shared__ __align__(16) uint32_t stage[2][S][NT];  // [buffer][plane][thread]: 4 digit bytes per thread
   const int tid = threadIdx.x;
   const long long nvec = cols >> 2;  // whole 4-element vectors
   uint32_t hm = 0;
   {
     long long v = tid;
-    for (; v + 768 < nvec; v += 1024) {  // four 256-bit loads in flight per thread
+    for (; v + 3 * NT < nvec; v += 4 * NT) {  // four 256-bit loads in flight per thread
       double a[16];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) ldg_nc_v4f64(x + 4 * (v + 256 * u), a[4 * u], a[4 * u + 1], a[4 * u + 2], a[4 * u + 3]);
+      for (int u = 0; u < 4; ++u) ldg_nc_v4f64(x + 4 * (v + NT * u), a[4 * u], a[4 * u + 1], a[4 * u + 2], a[4 * u + 3]);
 #pragma unroll
       for (int j = 0; j < 16; ++j) hm = max(hm, abs_hi_word(a[j]));
     }
-    for (; v < nvec; v += 256) {
+    for (; v < nvec; v += NT) {
       double a0, a1, a2, a3;
       ldg_nc_v4f64(x + 4 * v, a0, a1, a2, a3);
       hm = max(max(hm, abs_hi_word(a0)), max(abs_hi_word(a1), max(abs_hi_word(a2), abs_hi_word(a3))));
     }
-    for (long long c = 4 * nvec + tid; c < cols; c += 256) hm = max(hm, abs_hi_word(__ldg(x + c)));
+    for (long long c = 4 * nvec + tid; c < cols; c += NT) hm = max(hm, abs_hi_word(__ldg(x + c)));
   }
   hm = warp_max_u32(hm);
   if ((tid & 31) == 0) wmax[tid >> 5] = hm;
   __syncthreads();
   if (tid == 0) {
     uint32_t m = 0;
-    for (int i = 0; i < 8; ++i) m = max(m, wmax[i]);
+    for (int i = 0; i < NT / 32; ++i) m = max(m, wmax[i]);
     const int ee = scale_index_from_hi(m);
     e_sh = ee;
     e[row] = ee;
@@ -154,7 +158,7 @@ __global__ void __launch_bounds__(256) split_rows_v4_kernel(const double* __rest
   const double scale = pow2_double(63 - e_sh);
   int8_t* const prow = planes + row * pitch;
   int buf = 0;
-  for (long long c0 = 0; c0 < pitch; c0 += kRowChunk, buf ^= 1) {
+  for (long long c0 = 0; c0 < pitch; c0 += kChunk, buf ^= 1) {
     const long long c = c0 + 4 * tid;
     double a[4] = {0.0, 0.0, 0.0, 0.0};
     if (c + 3 < cols) {
@@ -176,9 +180,9 @@ __global__ void __launch_bounds__(256) split_rows_v4_kernel(const double* __rest
 #pragma unroll
     for (int t = 0; t < S; ++t) stage[buf][t][tid] = (t < 4) ? ph[3 - t] : pl[7 - t];
     __syncthreads();  // one barrier per chunk: buffer buf ^ 1 was last read before this barrier
-    // S planes x 1 KB: 64 sixteen-byte vectors per plane, whole runs per plane
-    for (int idx = tid; idx < S * 64; idx += 256) {
-      const int t = idx >> 6, v = idx & 63;
+    // S planes x 4 NT bytes: NT / 4 sixteen-byte vectors per plane, whole runs per plane
+    for (int idx = tid; idx < S * (NT / 4); idx += NT) {
+      const int t = idx / (NT / 4), v = idx % (NT / 4);
       const long long col = c0 + 16 * v;
       if (col < pitch)
         *reinterpret_cast<uint4*>(prow + t * plane_stride + col) = *reinterpret_cast<const uint4*>(&stage[buf][t][4 * v]);
@@ -278,8 +282,28 @@ cudaError_t launch_split_rows(const double* X, int64_t rows, int64_t cols, int64
   if (rows <= 0) return cudaSuccess;
   if (ld % 4 == 0 && ((uintptr_t)X & 31) == 0 && pitch % 16 == 0 && plane_stride % 16 == 0 &&
       ((uintptr_t)planes & 15) == 0) {
-    DFE_DISPATCH_S(s, (split_rows_v4_kernel<SS><<<(unsigned)rows, 256, 0, st>>>(X, cols, ld, e, planes, pitch,
-                                                                              plane_stride, status)));
+    // resident rows stay inside ~48 MB of L2: blocks per SM = 48 MB / (SMs x row bytes), 1..8, enforced by the
+    // dynamic shared memory each block asks for (it is not used); long rows take 512-thread blocks
+    int dev = 0, num_sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    const bool wide = cols >= 8192;
+    long long per_sm = (48ll << 20) / ((long long)num_sms * cols * 8);
+    per_sm = per_sm < 1 ? 1 : (per_sm > (wide ? 4 : 8) ? (wide ? 4 : 8) : per_sm);
+    const int pad = per_sm >= 8 ? 0 : (int)((200 * 1024) / per_sm) - (wide ? 2 * s * 2048 : 2 * s * 1024) - 1024;
+    cudaError_t err = cudaSuccess;
+    if (wide) {
+      DFE_DISPATCH_S(s, (err = cudaFuncSetAttribute(split_rows_v4_kernel<SS, 512>,
+                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, pad > 0 ? pad : 0),
+                         split_rows_v4_kernel<SS, 512><<<(unsigned)rows, 512, pad > 0 ? pad : 0, st>>>(
+                             X, cols, ld, e, planes, pitch, plane_stride, status)));
+    } else {
+      DFE_DISPATCH_S(s, (err = cudaFuncSetAttribute(split_rows_v4_kernel<SS, 256>,
+                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, pad > 0 ? pad : 0),
+                         split_rows_v4_kernel<SS, 256><<<(unsigned)rows, 256, pad > 0 ? pad : 0, st>>>(
+                             X, cols, ld, e, planes, pitch, plane_stride, status)));
+    }
+    if (err != cudaSuccess) return err;
     count_launch();
     return cudaGetLastError();
   }
