@@ -41,9 +41,9 @@ namespace dfe {
 static df_context g_default;
 
 // ---- optional per-kernel-class CUDA-event timing (df_profile_*; bench.py's roofline) ----
-enum ProfClass { kPSplit = 0, kPPassA, kPJGemv, kPUnpack, kPGemm5, kPSplitX, kPGemm6, kPReduce, kPGemm, kPNum };
+enum ProfClass { kPSplit = 0, kPPassA, kPJGemv, kPUnpack, kPGemm5, kPSplitX, kPGemm6, kPReduce, kPGemm, kPScreen, kPNum };
 static const char* const kProfNames[kPNum] = {"split",   "jk_pass_a", "jk_j_gemv", "jk_unpack_split", "gemm5_i8",
-                                              "jk_split_x", "gemm6_i8",  "jk_k_reduce", "emul_gemm_i8"};
+                                              "jk_split_x", "gemm6_i8",  "jk_k_reduce", "emul_gemm_i8", "jk_screen_mask"};
 struct ProfRec {
   int cls;
   cudaEvent_t e0, e1;
@@ -403,8 +403,11 @@ static int jk_impl(df_context& c, const double* Bp, int64_t nao, int64_t naux, c
     if (c.screening()) {
       const uint32_t* em = planned ? reinterpret_cast<const uint32_t*>(plan_b + PL.emax_off) : w.emax5;
       const uint32_t* tmx = planned ? reinterpret_cast<const uint32_t*>(plan_b + PL.tilemax_off) : w.tilemax;
-      DFE_CK(launch_jk_screen_mask(em, tmx, (int)nao, (int)naux, (int)qs0, nq, s, w.kmask,
-                                   reinterpret_cast<unsigned long long*>(w.status + 8), st));
+      {
+        ProfScope ps(kPScreen, st);
+        DFE_CK(launch_jk_screen_mask(em, tmx, (int)nao, (int)naux, (int)qs0, nq, s, w.kmask,
+                                     reinterpret_cast<unsigned long long*>(w.status + 8), st));
+      }
       kmask = w.kmask;
     }
 
