@@ -250,7 +250,8 @@ int df_debug_jk_build(const double* B_packed, int64_t nao, int64_t naux,
  *   bit 22     GEMM(5) N halves on multicast CTA pairs, never on MMA pairs
  *   bit 23     GEMM epilogue moves FP64 through the staged 16-byte path, never 256-bit accesses
  *   bit 24     df_emul_gemm keeps 128-column tiles at s <= 3 (default: 256 columns at s <= 2, 160 at s = 3)
- *   bit 25     no screening: every K block of GEMM(5) is written, loaded and multiplied */
+ *   bit 25     no screening: every K block of GEMM(5) is written, loaded and multiplied (plain builds and
+ *              plan creation; a planned build always screens, its plan may hold the active blocks only) */
 int df_debug_set_gemm_flags(int flags);
 
 /* Number of GPU kernels this library has launched in this process. */

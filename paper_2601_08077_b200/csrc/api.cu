@@ -399,8 +399,9 @@ static int jk_impl(df_context& c, const double* Bp, int64_t nao, int64_t naux, c
 
     // screening: the K blocks of GEMM(5)'s left operand that hold a
     // non-zero digit at s slices; the unpack pass writes and GEMM(5) reads only those
+    // (a planned build always screens: its plan may hold planes for the active blocks only)
     const uint32_t* kmask = nullptr;
-    if (c.screening()) {
+    if (planned || c.screening()) {
       const uint32_t* em = planned ? reinterpret_cast<const uint32_t*>(plan_b + PL.emax_off) : w.emax5;
       const uint32_t* tmx = planned ? reinterpret_cast<const uint32_t*>(plan_b + PL.tilemax_off) : w.tilemax;
       {
