@@ -797,3 +797,40 @@ def test_jk_dense_input_keeps_every_block(dfe, gpu_ws):
     run_jk(dfe, Bp, cfg.nao, cfg.naux, Cocc, cfg.nocc, D, 4)
     active, total = dfe.df_screen_stats()
     assert active == total == (cfg.naux * cfg.nao + 255) // 256
+
+
+def test_jk_screened_wide_mask_and_superblocks(dfe, gpu_ws):
+    """Screening where the mask of a 256-row block spans two 32-bit words (nao = 4200: 33 K blocks of
+    128 columns) and, separately, over several super-blocks (a minimum-size workspace: one 512-q block
+    per launch, masks indexed from each super-block's first q).  X bit for bit against the dense oracle."""
+    nao, naux, nocc, s = 4200, 6, 8, 3
+    Bp = G.make_B_packed_screened(nao, naux, seed=81, decay=0.05)
+    Cocc = G.make_C_occ(nao, nocc, seed=81)
+    D = G.make_density(Cocc)
+    dfe.df_screen_stats()
+    J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+    active, total = dfe.df_screen_stats()
+    assert total == ((naux * nao + 255) // 256) * 33 and 0 < active < 0.6 * total, (active, total)
+    K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
+    assert np.array_equal(X[:, :, :nocc], X_emu)
+    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    del Bp, X, X_emu
+
+    nao, naux, nocc, s = 300, 1100, 12, 4
+    Bp = G.make_B_packed_screened(nao, naux, seed=82, decay=0.5)
+    Cocc = G.make_C_occ(nao, nocc, seed=82)
+    D = G.make_density(Cocc)
+    small = dfe.Workspace(dfe.df_jk_workspace_bytes(nao, naux, nocc, s))
+    try:
+        dfe.df_screen_stats()
+        J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+        active, total = dfe.df_screen_stats()
+    finally:
+        small.close()
+        dfe.df_set_workspace(gpu_ws.view)
+    assert 0 < active < total
+    K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
+    assert np.array_equal(X[:, :, :nocc], X_emu)
+    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    J_ref, _ = O.df_jk_plain(Bp, nao, Cocc, D)
+    assert O.rel_frobenius(J, J_ref) <= 1e-12
