@@ -370,18 +370,18 @@ __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(co
     if (R >= nao) break;  // block-uniform
     // screening: bit B of the mask of the 256-row block of (q, R) -- lane = q in every warp, so the
     // ballot is the same in all warps and the branches below are block-uniform
+    const uint32_t hm = emax[(long long)R * naux + q];
+    const int e = scale_index_from_hi(hm);
+    if (lower && B == 0 && warp == 0 && q_ok) {  // the row's scale index is written whether or not its block is active
+      e5[(long long)(qg - q0) * nao + R] = e;
+      const int stt = status_from_hi(hm);
+      if (stt) atomicOr(status, stt);
+    }
     uint32_t act = 0xffffffffu;
     if (kmask) {
       const long long mb = ((long long)(q - q0) * nao + R) >> 8;
       act = __ballot_sync(0xffffffffu, q_ok && ((kmask[mb * mask_words + (B >> 5)] >> (B & 31)) & 1u));
       if (act == 0u && !do_j) continue;  // nothing to write, nothing to sum: the row is not even read
-    }
-    const uint32_t hm = emax[(long long)R * naux + q];
-    const int e = scale_index_from_hi(hm);
-    if (lower && B == 0 && warp == 0 && q_ok) {
-      e5[(long long)(qg - q0) * nao + R] = e;
-      const int stt = status_from_hi(hm);
-      if (stt) atomicOr(status, stt);
     }
     const double scale = pow2_double(63 - e);
     double x[16];

@@ -834,3 +834,40 @@ def test_jk_screened_wide_mask_and_superblocks(dfe, gpu_ws):
     assert O.rel_frobenius(K, K_emu) <= 1e-14
     J_ref, _ = O.df_jk_plain(Bp, nao, Cocc, D)
     assert O.rel_frobenius(J, J_ref) <= 1e-12
+
+
+def test_plan_of_screened_input_holds_every_scale_index(dfe, gpu_ws):
+    """A plan made from a screened B into a buffer full of garbage: the scale index of EVERY row (q, i) is
+    there (also of rows whose first K block is inactive and never written), and a planned build from it
+    gives the bits of the plain build."""
+    nao, naux, nocc, s = 768, 40, 24, 4  # a multiple of 256: a block of rows covers the same i for every q
+    Bp = G.make_B_packed_screened(nao, naux, seed=91, decay=0.6)
+    Cocc = G.make_C_occ(nao, nocc, seed=91)
+    D = G.make_density(Cocc)
+    Bd = dev(Bp)
+    plan = dfe.Plan.__new__(dfe.Plan)
+    plan.nao, plan.naux, plan.smax = nao, naux, 6
+    nbytes = dfe.df_jk_plan_bytes(nao, naux, 6)
+    plan.buf = torch.full((nbytes + 256,), 0x5A, dtype=torch.uint8, device=DEV)
+    off = (-plan.buf.data_ptr()) % 256
+    plan.view = plan.buf[off: off + nbytes]
+    rc = dfe.lib.df_jk_plan_create(Bd.data_ptr(), nao, naux, 6, plan.view.data_ptr(), nbytes, None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    active, total = dfe.df_screen_stats()
+    assert 0 < active < total
+    rows = naux * nao
+    r256 = lambda n: (n + 255) // 256 * 256
+    e5_off = r256(rows * 4) + r256(((nao + 31) // 32) * ((nao + 31) // 32 + 1) // 2 * naux * 4)
+    e5 = plan.view[e5_off: e5_off + rows * 4].view(torch.int32).cpu().numpy().reshape(naux, nao)
+    for q in range(naux):
+        Bq = O.unpack_sym(Bp[:, q], nao)
+        assert np.array_equal(e5[q], O.scale_index(np.max(np.abs(Bq), axis=1))), q
+    J = torch.empty((nao, nao), dtype=torch.float64, device=DEV)
+    K = torch.empty_like(J)
+    dfe.df_jk_build_slices(Bd, nao, naux, dev(Cocc), nocc, dev(D), s, J, K)
+    J2, K2 = torch.full_like(J, np.nan), torch.full_like(K, np.nan)
+    dfe.df_jk_build_planned_slices(plan, Bd, nao, naux, dev(Cocc), nocc, dev(D), s, J2, K2)
+    torch.cuda.synchronize()
+    assert torch.equal(J, J2) and torch.equal(K, K2)
+    assert O.rel_frobenius(K.cpu().numpy(), O.emul_df_k(Bp, nao, Cocc, s)) <= 1e-14
