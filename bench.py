@@ -246,7 +246,7 @@ def run_ours(args, cfg):
     else:
         nseq = NSEQ
         seq = G.make_scf_sequence(D0, nocc, NSEQ, cfg.seed)
-        sched = policy.schedule([eps * eps for eps, _, _ in seq])[:NSEQ]  # dE_rel,k := eps_k^2 (R11)
+        sched = policy.schedule_from_density_change([eps for eps, _, _ in seq])[:NSEQ]  # dE_rel,k := eps_k^2 (R11)
         tols = [t for _, t in sched]
     slices = [p.df_slices_for_tol(t) for t in tols]
     D_dev = [torch.from_numpy(Dk).to(dev) for _, Dk, _ in seq]

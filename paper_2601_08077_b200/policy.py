@@ -47,6 +47,19 @@ class AdaptiveTolerance:
         return self.tol
 
 
+def level_for_density_change(dD_rel: float) -> int:
+    """Emulation level for the NEXT iteration from the relative change of the density matrix,
+    ||D_k - D_{k-1}||_F / ||D_k||_F (the paper names a density-driven choice as future work).
+    The energy is stationary in the density, so its error is second order in the density error
+    (R11): dE_rel ~ dD_rel^2, looked up in Table 1 like a measured energy change."""
+    return level_for(dD_rel * dD_rel)
+
+
+def schedule_from_density_change(dD_rels):
+    """[(level, tol)] like `schedule`, driven by the density changes instead of the energy changes."""
+    return schedule([d * d for d in dD_rels])
+
+
 def schedule(dE_rels):
     """[(level, tol)] for iterations 0..len(dE_rels): iteration i+1 uses dE_rel of iteration i."""
     a = AdaptiveTolerance()

@@ -208,3 +208,19 @@ def test_context_entry_points_fail_loudly_without_a_device(dfe):
     assert dfe.lib.df_context_create(None, 1 << 20, C.byref(h)) == -1
     assert dfe.lib.df_context_jk_build(None, None, 1, 1, None, 1, None, 1e-6, None, None, None) == -1
     assert dfe.lib.df_context_destroy(None) == -1
+
+
+def test_density_change_schedule_is_the_energy_schedule_of_its_square():
+    """policy.schedule_from_density_change (future work in the paper): dE_rel ~ dD_rel^2,
+    then Table 1, monotone, lagged by one iteration, start level 4."""
+    from paper_2601_08077_b200 import policy
+
+    eps = [10.0 ** (-k / 2.0) for k in range(12)]
+    got = policy.schedule_from_density_change(eps)
+    assert got == policy.schedule([e * e for e in eps])
+    levels = [lv for lv, _ in got][:12]
+    assert levels == [4] * 7 + [3] * 3 + [2] * 2  # nominal splits 3 x 7, 4 x 3, 5 x 2 (DESIGN.md R11)
+    assert all(a >= b for a, b in zip(levels[:-1], levels[1:]))
+    assert policy.level_for_density_change(1e-2) == 4 and policy.level_for_density_change(1e-8) == 0
+    # the same levels as the oracle's independent statement of Table 1
+    assert [lv for lv, _ in O.adaptive_schedule([e * e for e in eps])][:12] == levels
