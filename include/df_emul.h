@@ -50,6 +50,7 @@ extern "C" {
 #define DF_ERR_DEVICE    -5  /* no CUDA device of compute capability 10.x     */
 #define DF_ERR_CUDA      -6  /* a CUDA runtime / driver call failed           */
 #define DF_ERR_ALIGN     -7  /* a pointer is not 16-byte aligned              */
+#define DF_ERR_TOO_LARGE -8  /* df_emul_gemm_static: the problem needs more scratch than the built-in array holds */
 
 #define DF_MODE_NOMINAL 0    /* tol -> s exactly as Table 1 */
 #define DF_MODE_GUARDED 1    /* one extra byte of margin (R7); default   */
@@ -147,6 +148,40 @@ int df_emul_gemm(const double* A, const double* B, double* C,
 int df_jk_build(const double* B_packed, int64_t nao, int64_t naux,
                 const double* C_occ, int64_t nocc, const double* D,
                 double tol, double* J, double* K, void* stream);
+
+/* ---- df_emul_gemm without a workspace: for callers that cannot allocate device memory ---- */
+
+/* df_emul_gemm (same arguments, same bits in C, tol -> s by the default context's policy mode) that needs
+ * NO workspace and allocates no device memory: no cudaMalloc / cudaFree / cudaMallocAsync, here or in
+ * anything it calls.  Every other compute entry point takes its scratch from a workspace the caller
+ * allocated; this one is for the callers that cannot allocate --
+ *   - an SCF driver that committed all of HBM (B, the plan, its own pool) at start-up,
+ *   - a callback invoked while its stream is being captured, where cudaMalloc is forbidden,
+ *   - a host thread next to other contexts' running builds, which cudaMalloc would stall
+ *     (it synchronises the whole device).
+ * The caller still owns and passes A, B and C (device, FP64, row-major, as for df_emul_gemm).
+ *
+ * The scratch (digit planes, scale indices, column maxima, status words) is a fixed array of
+ * df_emul_gemm_static_scratch_bytes() = 64 MiB inside the library's device image.  Every GPU on which
+ * the library is used holds that array until the process exits, called or not.
+ *   LIMIT   the problem must satisfy df_emul_gemm_workspace_bytes(m, n, k, s) <= 64 MiB, about
+ *           s (m + n) round_up(k, 32) bytes: 2048^3 up to s = 7, 1024 x 1024 x 3000 at s = 8.  Beyond it the
+ *           call returns DF_ERR_TOO_LARGE before touching the GPU; C is not written.
+ *   SHARED  all calls on one device use the same array.  Calls on ONE stream are ordered and safe.  Two
+ *           calls that may overlap on the GPU (two streams, two host threads) race on it and give
+ *           garbage: serialise them, or give the second caller a context with a workspace.  The array
+ *           keeps the previous call's contents; the call clears, in stream order, the one part that must
+ *           start at zero (the column maxima) and overwrites the rest, so a call never sees another's data.
+ *   SET-UP  the FIRST call on each device looks the array's address up on that device (with the device
+ *           current), clears its status words with a synchronous cudaMemset and creates a small host-side
+ *           tensor-map cache.  Make that first call outside any stream capture.
+ *   STATUS  DF_STATUS_* bits this entry point raises are kept in the array and not reported by
+ *           df_last_status(); validate the operands yourself if Inf/NaN can occur.
+ * Returns DF_ERR_TOO_LARGE as above, otherwise what df_emul_gemm returns. */
+int df_emul_gemm_static(const double* A, const double* B, double* C,
+                        int64_t m, int64_t n, int64_t k, double tol, void* stream);
+/* The size of that array in bytes (host only, no device needed). */
+int64_t df_emul_gemm_static_scratch_bytes(void);
 
 /* ---- plan: B split once for a whole SCF --- */
 

@@ -25,7 +25,7 @@ DF_MODE_NOMINAL, DF_MODE_GUARDED = 0, 1
 DF_STATUS_NONFINITE, DF_STATUS_RANGE = 1, 2
 _ERRORS = {
     -1: "DF_ERR_NULL", -2: "DF_ERR_DIM", -3: "DF_ERR_TOL", -4: "DF_ERR_WORKSPACE",
-    -5: "DF_ERR_DEVICE", -6: "DF_ERR_CUDA", -7: "DF_ERR_ALIGN",
+    -5: "DF_ERR_DEVICE", -6: "DF_ERR_CUDA", -7: "DF_ERR_ALIGN", -8: "DF_ERR_TOO_LARGE",
 }
 
 
@@ -48,6 +48,8 @@ _SIG = {
     "df_set_workspace": (_i32, [_vp, _i64]),
     "df_emul_gemm": (_i32, [_vp, _vp, _vp, _i64, _i64, _i64, _f64, _vp]),
     "df_emul_gemm_slices": (_i32, [_vp, _vp, _vp, _i64, _i64, _i64, _i32, _vp]),
+    "df_emul_gemm_static": (_i32, [_vp, _vp, _vp, _i64, _i64, _i64, _f64, _vp]),
+    "df_emul_gemm_static_scratch_bytes": (_i64, []),
     "df_jk_build": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _f64, _vp, _vp, _vp]),
     "df_jk_build_slices": (_i32, [_vp, _i64, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
     "df_jk_plan_bytes": (_i64, [_i64, _i64, _i32]),
@@ -275,6 +277,21 @@ def df_emul_gemm_slices(A, B, Cout, m, n, k, s, stream=None) -> None:
 
     _check(lib.df_emul_gemm_slices(_ptr(A, torch.float64), _ptr(B, torch.float64), _ptr(Cout, torch.float64),
                                    m, n, k, int(s), _stream(stream)), "df_emul_gemm_slices")
+
+
+def df_emul_gemm_static(A, B, Cout, m, n, k, tol, stream=None) -> None:
+    """df_emul_gemm for callers that cannot allocate device memory: no workspace is registered or
+    needed, the scratch is a 64 MiB array built into the library (include/df_emul.h).  Raises DFError
+    with code -8 (DF_ERR_TOO_LARGE) when the sizes need more than that; calls that may overlap on the
+    GPU must not share it."""
+    import torch
+
+    _check(lib.df_emul_gemm_static(_ptr(A, torch.float64), _ptr(B, torch.float64), _ptr(Cout, torch.float64),
+                                   m, n, k, float(tol), _stream(stream)), "df_emul_gemm_static")
+
+
+def df_emul_gemm_static_scratch_bytes() -> int:
+    return int(lib.df_emul_gemm_static_scratch_bytes())
 
 
 def df_jk_build(B_packed, nao, naux, C_occ, nocc, D, tol, J, K, stream=None) -> None:

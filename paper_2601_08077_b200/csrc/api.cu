@@ -6,6 +6,7 @@
 #include <stdint.h>
 
 #include <atomic>
+#include <mutex>
 #include <vector>
 
 #include "../../include/df_emul.h"
@@ -525,6 +526,49 @@ static int jk_impl(df_context& c, const double* Bp, int64_t nao, int64_t naux, c
   return DF_OK;
 }
 
+// ---------------------------------------------------------------------------
+// df_emul_gemm_static: df_emul_gemm for callers that have no device memory to give as a workspace
+// ---------------------------------------------------------------------------
+// Every other compute entry point carves its scratch (digit planes, scale indices, column maxima, status
+// words) from a workspace the CALLER allocated.  Some callers cannot allocate: an SCF driver that handed
+// all of HBM to B and its plan at start-up and has nothing left to give; a callback that runs while its
+// stream is being captured, where cudaMalloc is not allowed; a host thread that shares the device with
+// other contexts' builds, which a cudaMalloc would stall (it synchronises the whole device).  For them
+// the scratch of this one entry point is the array below, part of the library's device image: every GPU
+// that loads libdfemul holds these 64 MiB from the first use of the library until the process exits,
+// whether or not df_emul_gemm_static is ever called.
+constexpr int64_t kStaticScratchBytes = 64ll << 20;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+// In host code `g_static_scratch` is only a handle for the runtime's symbol calls, NOT a device address
+// (a kernel handed it would fault, or quietly use host memory where the GPU can reach it); and the
+// array has a different address on every device.  static_context() asks the runtime for the address
+// with the target device current and keeps it, with the tensor-map cache and SM count of that device,
+// in a context of its own.
+constexpr int kMaxStaticDevices = 64;
+static df_context g_static_ctx[kMaxStaticDevices];
+static std::mutex g_static_mu;
+
+// The context of the CURRENT device whose workspace is that device's copy of g_static_scratch.  Its
+// first call on a device sets the context up: cudaGetSymbolAddress, a synchronous cudaMemset of the
+// status words, a small host-side allocation (the tensor-map cache).  No device memory is allocated.
+static int static_context(df_context** out) {
+  const int dev = current_sm100_device();
+  if (dev < 0 || dev >= kMaxStaticDevices) return DF_ERR_DEVICE;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  df_context& c = g_static_ctx[dev];
+  if (!c.ws) {
+    void* ptr = nullptr;
+    if (cudaGetSymbolAddress(&ptr, g_static_scratch) != cudaSuccess || !ptr) {
+      cudaGetLastError();
+      return DF_ERR_CUDA;
+    }
+    if (const int rc = context_set_workspace(c, ptr, kStaticScratchBytes)) return rc;
+  }
+  *out = &c;
+  return DF_OK;
+}
+
 }  // namespace dfe
 
 // ===========================================================================
@@ -533,6 +577,25 @@ static int jk_impl(df_context& c, const double* Bp, int64_t nao, int64_t naux, c
 using namespace dfe;
 
 extern "C" {
+
+int64_t df_emul_gemm_static_scratch_bytes(void) { return kStaticScratchBytes; }
+
+int df_emul_gemm_static(const double* A, const double* B, double* C, int64_t m, int64_t n, int64_t k, double tol,
+                        void* stream) {
+  if (!A || !B || !C) return DF_ERR_NULL;
+  if (m <= 0 || n <= 0 || k <= 0 || k > (1ll << 30) || m >= (1ll << 31) || n > 65535ll * 32) return DF_ERR_DIM;
+  const int s = slices_for_tol(tol, g_default.mode);
+  if (s < 0) return s;
+  // the size check comes before any CUDA call: a problem that does not fit is refused, never truncated
+  if (carve_gemm(nullptr, m, n, k, s).bytes > kStaticScratchBytes) return DF_ERR_TOO_LARGE;
+  df_context* c = nullptr;
+  if (const int rc = static_context(&c)) return rc;
+  c->mode = g_default.mode;
+  // Nothing in the array has to start at zero except what the launch sequence clears itself, in stream
+  // order: the column maxima (cudaMemsetAsync inside launch_split_cols); planes, scale indices and the
+  // padding bytes of every plane row are rewritten in full by the split kernels of this call.
+  return emul_gemm_impl(*c, A, B, C, m, n, k, s, (cudaStream_t)stream);
+}
 
 int df_slices_for_tol(double tol, int mode) {
   if (mode != DF_MODE_NOMINAL && mode != DF_MODE_GUARDED) return DF_ERR_TOL;
