@@ -292,8 +292,9 @@ int df_debug_set_gemm_flags(int flags);
 /* Number of GPU kernels this library has launched in this process. */
 int64_t df_launch_count(void);
 
-/* Per-kernel-class device timing for the roofline report (bench.py); process-wide, for one stream at a
- * time (do not enable it while several contexts run concurrently).  While
+/* Per-kernel-class device timing for the roofline report (bench.py); process-wide: while it is on,
+ * the brackets of all contexts and host threads land in the same per-class sums (the records are
+ * guarded by a mutex; enable / read it from one thread).  While
  * enabled, every entry point brackets each kernel class it launches with a pair
  * of CUDA events on the caller's stream.  df_profile_read() SYNCHRONISES on the
  * recorded events, returns the summed milliseconds and the number of brackets

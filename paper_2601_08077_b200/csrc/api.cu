@@ -49,11 +49,13 @@ struct ProfRec {
   int cls;
   cudaEvent_t e0, e1;
 };
-static bool g_prof_on = false;
+static std::atomic<bool> g_prof_on{false};
+static std::mutex g_prof_mu;                // guards the two vectors: contexts may run on several host threads
 static std::vector<ProfRec> g_prof_recs;    // records of the current profiling window
 static std::vector<cudaEvent_t> g_prof_pool;  // recycled events
 static cudaEvent_t prof_event() {
   cudaEvent_t e;
+  std::lock_guard<std::mutex> lock(g_prof_mu);
   if (!g_prof_pool.empty()) {
     e = g_prof_pool.back();
     g_prof_pool.pop_back();
@@ -77,6 +79,7 @@ struct ProfScope {
   ~ProfScope() {
     if (on) {
       cudaEventRecord(r.e1, st);
+      std::lock_guard<std::mutex> lock(g_prof_mu);
       g_prof_recs.push_back(r);
     }
   }
@@ -195,7 +198,7 @@ static int emul_gemm_impl(df_context& c, const double* A, const double* B, doubl
 
   {
     ProfScope ps(kPSplit, st);
-    if (launch_split_rows(A, m, k, k, s, w.eA, w.pa, w.pitch, m * w.pitch, w.status, st) != cudaSuccess)
+    if (launch_split_rows(A, m, k, k, s, w.eA, w.pa, w.pitch, m * w.pitch, w.status, st, c.env.num_sms) != cudaSuccess)
       return DF_ERR_CUDA;
     if (launch_split_cols(B, k, n, s, w.cmax, w.eB, w.pb, w.pitch, n * w.pitch, w.status, st) != cudaSuccess)
       return DF_ERR_CUDA;
@@ -863,7 +866,7 @@ int df_debug_split_rows(const double* X, int64_t rows, int64_t cols, int s, int3
   if (const int rc = context_ready(g_default)) return rc;
   const int64_t pitch = plane_pitch(cols);
   if (launch_split_rows(X, rows, cols, cols, s, e, planes, pitch, rows * pitch, (int*)g_default.ws,
-                        (cudaStream_t)stream) != cudaSuccess)
+                        (cudaStream_t)stream, g_default.env.num_sms) != cudaSuccess)
     return DF_ERR_CUDA;
   return DF_OK;
 }
@@ -937,6 +940,7 @@ int df_profile_read(float* ms_by_class, int* count_by_class) {
     count_by_class[i] = 0;
   }
   int rc = DF_OK;
+  std::lock_guard<std::mutex> lock(g_prof_mu);
   for (ProfRec& r : g_prof_recs) {
     float ms = 0.f;
     if (cudaEventSynchronize(r.e1) != cudaSuccess || cudaEventElapsedTime(&ms, r.e0, r.e1) != cudaSuccess)

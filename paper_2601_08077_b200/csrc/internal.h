@@ -69,9 +69,10 @@ bool encode_tensor_map(void* map, int dtype, int rank, const void* base, const u
 
 // ---- split.cu -------------------------------------------------------------
 // rows x cols FP64 (leading dimension ld) -> e[rows], planes[t][rows][pitch].
+// num_sms: LaunchEnv::num_sms of the calling context (0: the launcher asks the runtime).
 cudaError_t launch_split_rows(const double* X, int64_t rows, int64_t cols, int64_t ld, int s, int32_t* e,
                               int8_t* planes, int64_t pitch, int64_t plane_stride, int* status,
-                              cudaStream_t st);
+                              cudaStream_t st, int num_sms = 0);
 // k x n FP64 row-major -> e[n] (scratch cmax[n] uint32), planes[t][n][pitch] transposed.
 cudaError_t launch_split_cols(const double* X, int64_t k, int64_t n, int s, uint32_t* cmax, int32_t* e,
                               int8_t* planes, int64_t pitch, int64_t plane_stride, int* status,

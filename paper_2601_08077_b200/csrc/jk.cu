@@ -331,6 +331,12 @@ __global__ void __launch_bounds__(256) jk_j_reduce_kernel(const double* __restri
 // of tiles in flight, and with it the L2 working set, small (8 rows: 11.2 / 16.9 ms at s = 4 / 6
 // against 10.5 / 14.3 ms).  Four resident blocks per SM up to s = 4, three above (measured both ways).
 constexpr int kUnpackRows = 2;
+// Row r stages through buffer r & 1 and is protected by ONE barrier per processed row; a row that the
+// screening mask skips (`continue` below) skips its barrier too.  With two rows every buffer is used
+// once per block, so that is safe; with three or more, row r + 2 could overwrite buffer r & 1 while
+// other warps still copy row r out of it.  Drive the buffer parity and the barrier by a count of the
+// processed rows before raising this.
+static_assert(kUnpackRows <= 2, "jk_unpack_split_kernel: skipped rows skip the barrier that guards the double buffer");
 constexpr int kUnpackPitch = 144;  // staging row: 128 bytes + 16 (conflict-free 16-byte stores by 8 lanes)
 template <int S>
 __global__ void __launch_bounds__(256, S <= 4 ? 4 : 3) jk_unpack_split_kernel(const double* __restrict__ Bp, int nao, int naux,

@@ -278,28 +278,37 @@ __global__ void __launch_bounds__(256) split_cols_tile_kernel(const double* __re
 
 cudaError_t launch_split_rows(const double* X, int64_t rows, int64_t cols, int64_t ld, int s, int32_t* e,
                               int8_t* planes, int64_t pitch, int64_t plane_stride, int* status,
-                              cudaStream_t st) {
+                              cudaStream_t st, int num_sms) {
   if (rows <= 0) return cudaSuccess;
   if (ld % 4 == 0 && ((uintptr_t)X & 31) == 0 && pitch % 16 == 0 && plane_stride % 16 == 0 &&
       ((uintptr_t)planes & 15) == 0) {
     // resident rows stay inside ~48 MB of L2: blocks per SM = 48 MB / (SMs x row bytes), 1..8, enforced by the
     // dynamic shared memory each block asks for (it is not used); long rows take 512-thread blocks
-    int dev = 0, num_sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (num_sms <= 0) {  // callers without a context (a context passes the count of its device)
+      int dev = 0;
+      num_sms = 148;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
     const bool wide = cols >= 8192;
     long long per_sm = (48ll << 20) / ((long long)num_sms * cols * 8);
     per_sm = per_sm < 1 ? 1 : (per_sm > (wide ? 4 : 8) ? (wide ? 4 : 8) : per_sm);
-    const int pad = per_sm >= 8 ? 0 : (int)((200 * 1024) / per_sm) - (wide ? 2 * s * 2048 : 2 * s * 1024) - 1024;
+    const int used = (wide ? 2 * s * 2048 : 2 * s * 1024) + 1024;
+    const int pad = per_sm >= 8 ? 0 : (int)((200 * 1024) / per_sm) - used;
+    // The attribute belongs to the kernel instantiation, not to a context or stream: it is always set to
+    // the largest request any call can make (one block per SM), the same value from every host thread,
+    // and only the launch's own dynamic size varies -- two contexts with different `cols` cannot make
+    // each other's launch fail.
+    const int max_pad = 200 * 1024 - used;
     cudaError_t err = cudaSuccess;
     if (wide) {
       DFE_DISPATCH_S(s, (err = cudaFuncSetAttribute(split_rows_v4_kernel<SS, 512>,
-                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, pad > 0 ? pad : 0),
+                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, max_pad),
                          split_rows_v4_kernel<SS, 512><<<(unsigned)rows, 512, pad > 0 ? pad : 0, st>>>(
                              X, cols, ld, e, planes, pitch, plane_stride, status)));
     } else {
       DFE_DISPATCH_S(s, (err = cudaFuncSetAttribute(split_rows_v4_kernel<SS, 256>,
-                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, pad > 0 ? pad : 0),
+                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, max_pad),
                          split_rows_v4_kernel<SS, 256><<<(unsigned)rows, 256, pad > 0 ? pad : 0, st>>>(
                              X, cols, ld, e, planes, pitch, plane_stride, status)));
     }

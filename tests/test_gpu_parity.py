@@ -742,6 +742,59 @@ def test_two_contexts_two_streams_concurrent(dfe, gpu_ws):
             c.close()
 
 
+def test_two_contexts_two_host_threads(dfe, gpu_ws):
+    """Two contexts driven from two HOST threads (ctypes releases the GIL inside a call), same slice
+    count, different contraction lengths: the row split's occupancy cap differs per call (the dynamic
+    shared memory it asks for depends on `cols`), while the kernel attribute it is checked against is
+    one per instantiation in the whole process.  Every call must succeed and give the serial bits,
+    also with the per-class profiler recording from both threads."""
+    import threading
+
+    s = 4
+    shapes = [(96, 64, 16384), (96, 64, 4096)]  # 148 SMs x cols x 8 bytes: 2 and 8 resident rows per SM
+    ops = []
+    for i, (m, n, k) in enumerate(shapes):
+        A, B = G.make_gemm_inputs(m, n, k, seed=70 + i)
+        Ad, Bd = dev(A), dev(B)
+        Cser = torch.empty((m, n), dtype=torch.float64, device=DEV)
+        dfe.df_emul_gemm_slices(Ad, Bd, Cser, m, n, k, s)
+        ops.append((Ad, Bd, Cser))
+    torch.cuda.synchronize()
+    ctxs = [dfe.Context(dfe.df_emul_gemm_workspace_bytes(m, n, k, s)) for m, n, k in shapes]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    errors = []
+
+    def work(i):
+        m, n, k = shapes[i]
+        Ad, Bd, Cser = ops[i]
+        try:
+            with torch.cuda.stream(streams[i]):
+                for _ in range(200):
+                    C2 = torch.full_like(Cser, np.nan)
+                    ctxs[i].emul_gemm_slices(Ad, Bd, C2, m, n, k, s)
+                streams[i].synchronize()
+                if not torch.equal(C2, Cser):
+                    errors.append((i, "bits differ"))
+        except Exception as exc:  # DFError of a failed launch
+            errors.append((i, repr(exc)))
+
+    dfe.df_profile_enable(True)
+    try:
+        threads = [threading.Thread(target=work, args=(i,)) for i in (0, 1)]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        torch.cuda.synchronize()
+        prof = dfe.df_profile_read()
+    finally:
+        dfe.df_profile_enable(False)
+        for c in ctxs:
+            c.close()
+    assert not errors, errors
+    assert prof["emul_gemm_i8"][1] == 400 and prof["split"][1] == 400, prof
+
+
 @pytest.mark.parametrize("s", [3, 4, 6])
 def test_jk_screened_input_bit_exact(dfe, gpu_ws, s):
     """on a B that decays away from the diagonal the
