@@ -60,6 +60,18 @@ def schedule_from_density_change(dD_rels):
     return schedule([d * d for d in dD_rels])
 
 
+def measured_density_changes(densities):
+    """dD_rel,k = ||D_k - D_{k-1}||_F / ||D_k||_F of consecutive density matrices (NumPy arrays), the
+    input of schedule_from_density_change.  Iteration 0 has no predecessor: its change is reported as
+    1.0, which keeps the start level."""
+    import numpy as np
+
+    out = [1.0]
+    for prev, cur in zip(densities[:-1], densities[1:]):
+        out.append(float(np.linalg.norm(cur - prev) / np.linalg.norm(cur)))
+    return out
+
+
 def schedule(dE_rels):
     """[(level, tol)] for iterations 0..len(dE_rels): iteration i+1 uses dE_rel of iteration i."""
     a = AdaptiveTolerance()

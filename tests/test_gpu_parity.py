@@ -742,6 +742,38 @@ def test_two_contexts_two_streams_concurrent(dfe, gpu_ws):
             c.close()
 
 
+@pytest.mark.parametrize("rule", ["energy_proxy", "density_change"])
+def test_scf_sequence_every_step_within_its_tol(dfe, gpu_ws, rule):
+    """The 12-step sequence of BASELINE.json configs[2] at a reduced size, under the schedule bench.py
+    times (R11: dE_rel,k := eps_k^2) and under the density-change rule fed with the MEASURED
+    ||D_k - D_{k-1}|| / ||D_k||: at EVERY step, not only the last, K is within the
+    tolerance the schedule chose for that step of the oracle's plain FP64 K, and J within 1e-12."""
+    from paper_2601_08077_b200 import policy
+
+    nao, naux, nocc, seed = 160, 600, 24, 17
+    Bp = G.make_B_packed(nao, naux, seed=seed)
+    D0 = G.make_density(G.make_C_occ(nao, nocc, seed=seed))
+    seq = G.make_scf_sequence(D0, nocc, 12, seed)
+    if rule == "energy_proxy":
+        sched = policy.schedule([eps * eps for eps, _, _ in seq])[:12]
+    else:
+        sched = policy.schedule_from_density_change(policy.measured_density_changes([Dk for _, Dk, _ in seq]))[:12]
+    Bd = dev(Bp)
+    J = torch.empty((nao, nao), dtype=torch.float64, device=DEV)
+    K = torch.empty_like(J)
+    used = []
+    for (eps, Dk, Ck), (level, tol) in zip(seq, sched):
+        dfe.df_jk_build(Bd, nao, naux, dev(Ck), nocc, dev(Dk), tol, J, K)
+        torch.cuda.synchronize()
+        J_ref, K_ref = O.df_jk_plain(Bp, nao, Ck, Dk)
+        assert O.rel_frobenius(J.cpu().numpy(), J_ref) <= 1e-12, (rule, eps)
+        err = O.rel_frobenius(K.cpu().numpy(), K_ref)
+        assert err <= tol, (rule, eps, level, tol, err)
+        used.append(dfe.df_slices_for_tol(tol))
+    assert used == sorted(used) and used[0] < used[-1]  # precision only ever tightens, and it does
+    assert dfe.df_last_status() == 0
+
+
 def test_two_contexts_two_host_threads(dfe, gpu_ws):
     """Two contexts driven from two HOST threads (ctypes releases the GIL inside a call), same slice
     count, different contraction lengths: the row split's occupancy cap differs per call (the dynamic

@@ -224,3 +224,26 @@ def test_density_change_schedule_is_the_energy_schedule_of_its_square():
     assert policy.level_for_density_change(1e-2) == 4 and policy.level_for_density_change(1e-8) == 0
     # the same levels as the oracle's independent statement of Table 1
     assert [lv for lv, _ in O.adaptive_schedule([e * e for e in eps])][:12] == levels
+
+
+def test_measured_density_changes_of_the_synthetic_sequence():
+    """The step-to-step change of D_k = D* + eps_k S_k (unit-norm S_k, eps_k = 10^(-k/2)) is
+    sqrt(eps_k^2 + eps_{k-1}^2 - 2 eps_k eps_{k-1} <S_k, S_{k-1}>) / ||D_k||: close to
+    sqrt(eps_k^2 + eps_{k-1}^2) / ||D*|| for independent S_k, and NOT eps_k itself; the schedule it
+    drives is monotone and never looser than level 4."""
+    import numpy as np
+
+    from df_inputs import generators as G
+    from paper_2601_08077_b200 import policy
+
+    nao, nocc = 60, 8
+    C0 = G.make_C_occ(nao, nocc, 5)
+    D0 = G.make_density(C0)
+    seq = G.make_scf_sequence(D0, nocc, 12, 5)
+    dD = policy.measured_density_changes([Dk for _, Dk, _ in seq])
+    assert dD[0] == 1.0 and len(dD) == 12
+    for k in range(1, 12):
+        want = np.hypot(seq[k][0], seq[k - 1][0]) / np.linalg.norm(D0)
+        assert 0.8 * want <= dD[k] <= 1.25 * want, (k, dD[k], want)
+    levels = [lv for lv, _ in policy.schedule_from_density_change(dD)][:12]
+    assert levels[0] == levels[1] == 4 and all(a >= b for a, b in zip(levels[:-1], levels[1:]))
