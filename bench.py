@@ -36,7 +36,9 @@ NSEQ = 12
 METRIC = "df_jk_builds_per_s"
 UNIT = "builds/s"
 CONFIG_INDEX = {"tiny": 0, "gemm": 1, "medium": 2, "large": 3, "largest": 4}  # BASELINE.json configs[i]
-NCU_TABLE = os.path.join("profiles", "r02_ncu_kernels.csv")  # per-kernel ncu counters by slice count
+NCU_TABLE = os.path.join("profiles", "ncu_kernels.csv")  # per-kernel ncu counters by slice count (--ncu-raw writes it)
+NOMINAL_INT8_TOPS = 4500.0  # dense INT8 tensor peak of a B200 (2 x the nominal 2.25 PFLOP/s bf16)
+CSRC = os.path.join("paper_2601_08077_b200", "csrc")
 
 
 def flops_per_build(cfg):
@@ -54,16 +56,17 @@ def int8_ops_per_build(cfg, s):
     return pairs * g5, pairs * g6
 
 
-def unpack_bytes_per_build(cfg, s, with_j=True):
-    """Algorithmic HBM bytes of the unpack + split pass: packed B read once,
-    s digit planes of naux * nao rows of round_up(nao, 128) bytes written, and the chunk partials of
-    Eq. 4 (one double per packed pair and 32-q chunk) written by a plain build."""
+def unpack_bytes_per_build(cfg, s, design=False):
+    """HBM bytes of the unpack + split pass.  Algorithmic (23.06 + 5.76 s GB at
+    config 3): packed B read once, s digit planes of naux * nao rows of nao bytes written.
+    design=True: what this layout moves on top of that -- rows padded to whole 128-byte lines
+    (round_up(nao, 128)) and the chunk partials of Eq. 4 a plain build writes (one double per packed
+    pair and 32-q chunk)."""
     npair = cfg.nao * (cfg.nao + 1) // 2
+    if not design:
+        return 8.0 * npair * cfg.naux + float(s) * cfg.naux * cfg.nao * cfg.nao
     pitch = (cfg.nao + 127) // 128 * 128
-    b = 8.0 * npair * cfg.naux + float(s) * cfg.naux * cfg.nao * pitch
-    if with_j:
-        b += 8.0 * npair * ((cfg.naux + 31) // 32)
-    return b
+    return 8.0 * npair * cfg.naux + float(s) * cfg.naux * cfg.nao * pitch + 8.0 * npair * ((cfg.naux + 31) // 32)
 
 
 def measured_peaks():
@@ -75,16 +78,99 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
 
 
+def kernel_sources_sha16():
+    """Hash of the kernel sources (every file of csrc/, names and bytes): the ncu table records the
+    one it was captured from, and its counters are quoted only while the two agree."""
+    import hashlib
+
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, CSRC)
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            h.update(name.encode())
+            with open(os.path.join(d, name), "rb") as f:
+                h.update(f.read())
+    return h.hexdigest()[:16]
+
+
 def ncu_table():
-    """{(kernel class, s): row} from the committed ncu captures (profiles/r02_ncu_kernels.csv; the
-    commands that made it are in profiles/r02_ncu_summary.md).  Counters, not timings."""
+    """({(kernel class, s): row}, stale) from the committed ncu capture (profiles/ncu_kernels.csv,
+    written by `bench.py --ncu-raw`; the commands are in profiles/r03_ncu_summary.md).  Counters, not
+    timings.  stale: the kernels' sources have changed since the capture."""
     path = os.path.join(ROOT, NCU_TABLE)
     out = {}
     if os.path.exists(path):
         with open(path) as f:
             for row in csv.DictReader(f):
                 out[(row["kernel_class"], int(row["s"]))] = row
-    return out
+    here = kernel_sources_sha16()
+    stale = any(r.get("sources_sha16") != here for r in out.values())
+    return out, stale
+
+
+NCU_COLUMNS = (  # column of profiles/ncu_kernels.csv <- metric of `ncu --page raw --csv --print-units base`
+    ("duration_ms", "gpu__time_duration.sum", 1e-6),
+    ("dram_read_bytes", "dram__bytes_read.sum", 1.0),
+    ("dram_write_bytes", "dram__bytes_write.sum", 1.0),
+    ("tensor_pipe_active_pct", "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_elapsed", 1.0),
+    ("l2_hit_pct", "lts__t_sector_hit_rate.pct", 1.0),
+    ("warp_inst", "smsp__inst_executed.sum", 1.0),
+    ("issue_active_pct", "smsp__issue_active.avg.pct", 1.0),
+    ("regs", "launch__registers_per_thread", 1.0),
+)
+
+
+def distill_ncu_raw(paths):
+    """profiles/ncu_kernels.csv from `ncu -i X.ncu-rep --page raw --csv --print-units base` exports of a
+    bench.py run: the first launch of every (kernel class, slice count).  A GEMM launch takes the slice
+    count of the unpack launch before it (a build runs unpack<S>, GEMM(5), GEMM(6) in that order);
+    GEMM(5) is the persistent grid (one CTA per SM), GEMM(6) the other."""
+    import re
+
+    def num(x):
+        try:
+            return float(str(x).replace(",", ""))
+        except ValueError:
+            return None
+
+    rows, seen = [], set()
+    sha = kernel_sources_sha16()
+    for path in paths:
+        with open(path, newline="") as f:
+            lines = [ln for ln in f if ln.startswith('"')]  # ncu prints ==PROF== lines before the table
+        s_now = None
+        for r in csv.DictReader(lines):
+            if num(r.get("ID", "")) is None:
+                continue  # the units row
+            name = r.get("Kernel Name", "")
+            grid = 1
+            for g in re.findall(r"\d+", r.get("Grid Size", "1")):
+                grid *= int(g)
+            m = re.search(r"(jk_unpack_split|split_rows_v4|split_cols_tile|jk_split_x)_kernel<(\d+)", name)
+            if m and m.group(1) == "jk_unpack_split":
+                s_now = int(m.group(2))
+                key = ("jk_unpack_split", s_now)
+            elif m:
+                key = (m.group(1), int(m.group(2)))
+            elif "gemm_i8_kernel" in name and s_now is not None:
+                key = ("gemm5_i8" if grid <= 160 else "gemm6_i8", s_now)
+            else:
+                continue
+            if key in seen:
+                continue
+            seen.add(key)
+            row = {"kernel_class": key[0], "s": key[1], "kernel": name.split("(")[0], "grid": grid, "sources_sha16": sha}
+            for col, metric, scale in NCU_COLUMNS:
+                v = num(r.get(metric, ""))
+                row[col] = "" if v is None else v * scale
+            rows.append(row)
+    rows.sort(key=lambda r: (r["s"], r["kernel_class"]))
+    out = os.path.join(ROOT, NCU_TABLE)
+    with open(out, "w", newline="") as f:
+        w = csv.DictWriter(f, fieldnames=["kernel_class", "s", "kernel", "grid"] + [c for c, _, _ in NCU_COLUMNS] + ["sources_sha16"])
+        w.writeheader()
+        w.writerows(rows)
+    print(f"{out}: {len(rows)} rows, sources {sha}")
 
 
 def traffic_for_mix(table, classes, used):
@@ -427,17 +513,38 @@ def run_ours(args, cfg):
     ms6, n6 = prof["gemm6_i8"]
     msu, nu = prof["jk_unpack_split"]
     peaks, peak_kind = measured_peaks()
-    table = ncu_table()
-    # INT8 dense peak = measured bf16 peak x the nominal INT8:bf16 ratio (4.5 : 2.25 PFLOP/s);
-    # the GEMMs run inside a long step, so the sustained figure applies.
+    table, table_stale = ncu_table()
+    if table_stale:  # counters of other kernels than the ones timed here are not quoted
+        table = {}
+    # The roofline's peak is a PROXY for the dense INT8 peak: the measured bf16 peak x the nominal
+    # INT8:bf16 ratio (4.5 : 2.25 PFLOP/s); the GEMMs run inside a long step, so the sustained figure
+    # applies.  It was measured at the bf16 GEMM's power-capped clock, below the clock these kernels
+    # run at, so `frac` flatters: `frac_of_nominal` (4.5 POP/s) and `frac_of_probe` (this library's own
+    # back-to-back MMA issue rate, measured in this run) are the stricter readings, and the ncu
+    # tensor-pipe-active percentages are the clock-independent one.
     peak_tops = 2.0 * peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
     achieved = (ops5 + ops6) / ((ms5 + ms6) / 1e3) / 1e12
     ubytes = sum(unpack_bytes_per_build(cfg, s) for s in used)
+    ubytes_design = sum(unpack_bytes_per_build(cfg, s, design=True) for s in used)
     hbm_achieved = ubytes / (msu / 1e3) / 1e9 if msu else None
 
     def pipe_pct(cls):
         v = {str(s): float(table[(cls, s)]["tensor_pipe_active_pct"]) for s in sorted(set(used)) if (cls, s) in table}
         return v or None
+
+    # one build per distinct slice count, timed alone: lets runs with different --steps windows compare
+    by_s = {}
+    for sl in sorted(set(slices)):
+        k = slices.index(sl)
+        step(k, True)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(3):
+            step(k, True)
+        e1.record()
+        torch.cuda.synchronize()
+        by_s[str(sl)] = e0.elapsed_time(e1) / 3
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -456,7 +563,8 @@ def run_ours(args, cfg):
         "clocks": clocks,
         "roofline": {"bound": "tensor", "kernel": "gemm_i8_kernel (GEMM(5) + GEMM(6) launches)",
                      "achieved": achieved, "peak": peak_tops, "unit": "TOP/s", "frac": achieved / peak_tops,
-                     "peak_source": f"2 x bf16_tflops_sustained of MEASURED_PEAKS.json ({peak_kind})",
+                     "peak_source": f"PROXY for the dense INT8 peak: 2 x bf16_tflops_sustained of MEASURED_PEAKS.json ({peak_kind})",
+                     "nominal_int8_tops": NOMINAL_INT8_TOPS, "frac_of_nominal": achieved / NOMINAL_INT8_TOPS,
                      "achieved_gemm5": ops5 / (ms5 / 1e3) / 1e12 if ms5 else None,
                      "achieved_gemm6": ops6 / (ms6 / 1e3) / 1e12 if ms6 else None,
                      "int8_probe_tops": int8_probe_tops, "frac_of_probe": achieved / int8_probe_tops,
@@ -465,7 +573,7 @@ def run_ours(args, cfg):
                      "traffic": traffic_for_mix(table, ("gemm5_i8", "gemm6_i8"), used),
                      "traffic_unit": "dram read + write bytes per launch, mean over the two GEMM launches of the timed "
                                      "steps' slice counts",
-                     "traffic_source": NCU_TABLE if table else None,
+                     "traffic_source": NCU_TABLE if table else None, "traffic_stale": table_stale,
                      "ncu_tensor_pipe_active_pct_gemm5": pipe_pct("gemm5_i8"),
                      "ncu_tensor_pipe_active_pct_gemm6": pipe_pct("gemm6_i8")},
         "roofline_hbm": {"bound": "hbm", "kernel": "jk_unpack_split_kernel (+ the chunk partials of Eq. 4)",
@@ -473,10 +581,15 @@ def run_ours(args, cfg):
                          "frac": hbm_achieved / peaks["hbm_gbs"] if hbm_achieved else None,
                          "peak_source": f"hbm_gbs of MEASURED_PEAKS.json ({peak_kind}; copy bandwidth)",
                          "launches": nu, "avg_launch_ms": msu / max(1, nu), "share_of_step": msu / ms_prof,
+                         "bytes": "algorithmic (SURVEY.md 8(d)): packed B read once + s planes of nao-byte rows written",
+                         "design_bytes_frac": (ubytes_design / (msu / 1e3) / 1e9 / peaks["hbm_gbs"]) if msu else None,
+                         "design_bytes_note": "with the layout's own extra bytes: rows padded to 128-byte lines, Eq. 4 chunk partials",
                          "traffic": traffic_for_mix(table, ("jk_unpack_split",), used),
-                         "traffic_source": NCU_TABLE if table else None},
+                         "traffic_source": NCU_TABLE if table else None, "traffic_stale": table_stale},
         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items() if v[1]},
         "profiled_ms_per_step": ms_prof / args.steps,
+        "ms_per_build_by_slices": by_s,
+        "kernel_sources_sha16": kernel_sources_sha16(),
         "screening": screening,
     }
     if density_schedule is not None:
@@ -672,7 +785,12 @@ def main():
                     help="decay of a Schwarz-like fall-off exp(-decay |i - j|) of B (0: the configs' unstructured B)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-level0", dest="level0", action="store_false")
+    ap.add_argument("--ncu-raw", dest="ncu_raw", nargs="+", default=None,
+                    help="no run: distil `ncu --page raw --csv --print-units base` exports into " + NCU_TABLE)
     args = ap.parse_args()
+    if args.ncu_raw:
+        distill_ncu_raw(args.ncu_raw)
+        return
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.config == "gemm":
         if args.impl == "reference":

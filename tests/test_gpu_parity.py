@@ -742,6 +742,43 @@ def test_two_contexts_two_streams_concurrent(dfe, gpu_ws):
             c.close()
 
 
+@pytest.mark.parametrize("s,nocc", [(3, 250), (4, 250), (3, 256), (4, 256)])
+def test_gemm6_int32_guard_worst_case_digits_exact(dfe, gpu_ws, s, nocc):
+    """The INT32 guard of GEMM(6)'s q-groups (R4/R5: s |g| nocc 2^14 < 2^31), pinned WITHOUT the
+    oracle's grouping rule: every X^q_ia is the same value v whose balanced digits are the most
+    negative a scaled operand can have, (-126, -128, ..., -128) (|x| 2^-e < 127/128 excludes a top
+    digit beyond +-126 when the rest is -128), so every INT32 weight sum of every group is within 1 %
+    of the largest a group of that length can reach: a group 2 % too long wraps around.  Whatever the
+    grouping, K_ij = naux nocc sum_{t+u<=s+1} d_t d_u 2^(2e+2-8(t+u)), computed here in Python integers
+    and exactly representable in FP64 at every partial sum -- K must equal it bit for bit."""
+    nao, naux = 72, 600
+    d = [-126] + [-128] * (s - 1)
+    v = sum(dt * 256 ** (s - 1 - t) for t, dt in enumerate(d))  # an integer of 8 s bits: x = v, scale index 8 s - 1
+    e = 8 * s - 1
+    assert 0.5 <= abs(v) / 2.0 ** e < 127.0 / 128.0
+    # B^q_i0 = v for every i and q, every other element 0; C_0a = 1, every other element 0  =>  X^q_ia = v
+    Bp = np.zeros((nao * (nao + 1) // 2, naux))
+    Bp[[i * (i + 1) // 2 for i in range(nao)], :] = float(v)
+    Cocc = np.zeros((nao, nocc)); Cocc[0, :] = 1.0
+    D = np.eye(nao)
+    J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
+    assert ng >= 2 and np.array_equal(X[:, :, :nocc], np.full((naux, nao, nocc), float(v)))
+    assert np.array_equal(e6, np.full((ng, nao), e))
+    # per element: sum over the retained pairs, as an exact integer multiple of 2^(2e + 2 - 8(s + 1))
+    unit = 2 * e + 2 - 8 * (s + 1)
+    terms = [d[t] * d[u] * 2 ** (8 * (s + 1 - (t + 1) - (u + 1))) for t in range(s) for u in range(s) if t + u + 2 <= s + 1]
+    total = sum(terms) * naux * nocc
+    # every term is a multiple of 2^tz and the total below 2^(53 + tz): every partial sum, in any order, is exact
+    tz = min((x & -x).bit_length() - 1 for x in terms)
+    assert (total >> tz) < 2 ** 53 and unit >= 0
+    # the worst weight sum of a maximal group really is at the edge of INT32: above 98 % of 2^31
+    worst_pairs = max(sum(d[t] * d[w - 2 - t] for t in range(s) if 0 <= w - 2 - t < s) for w in range(2, s + 2))
+    assert 0.98 * 2 ** 31 <= worst_pairs * (dfe.df_kflush(s) // nocc) * nocc < 2 ** 31
+    assert np.array_equal(K, np.full((nao, nao), float(total * 2 ** unit)))
+    assert np.array_equal(K, O.emul_df_k(Bp, nao, Cocc, s))
+    assert dfe.df_last_status() == 0
+
+
 @pytest.mark.parametrize("rule", ["energy_proxy", "density_change"])
 def test_scf_sequence_every_step_within_its_tol(dfe, gpu_ws, rule):
     """The 12-step sequence of BASELINE.json configs[2] at a reduced size, under the schedule bench.py
