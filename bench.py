@@ -16,6 +16,7 @@ from __future__ import annotations
 
 import argparse
 import csv
+import dataclasses
 import json
 import os
 import statistics
@@ -115,7 +116,8 @@ NCU_COLUMNS = (  # column of profiles/ncu_kernels.csv <- metric of `ncu --page r
     ("tensor_pipe_active_pct", "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_elapsed", 1.0),
     ("l2_hit_pct", "lts__t_sector_hit_rate.pct", 1.0),
     ("warp_inst", "smsp__inst_executed.sum", 1.0),
-    ("issue_active_pct", "smsp__issue_active.avg.pct", 1.0),
+    ("tma_load_bytes", "l1tex__m_xbar2l1tex_read_bytes_mem_global_op_tma_ld.sum", 1.0),
+    ("inst_issued_pct", "sm__inst_issued.avg.pct_of_peak_sustained_active", 1.0),
     ("regs", "launch__registers_per_thread", 1.0),
 )
 
@@ -318,9 +320,19 @@ def run_ours(args, cfg):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    nao, naux, nocc = cfg.nao, cfg.naux, cfg.nocc
-    # ---- inputs (synthetic, seeded).  With N ranks every rank owns one
-    # q-shard of `naux` auxiliary functions of an N*naux basis (weak scaling).
+    nao, nocc = cfg.nao, cfg.nocc
+    # ---- inputs (synthetic, seeded).  With N ranks the SAME build (the config's
+    # nao, naux, nocc) is q-sharded: rank r owns the 512-aligned range shard_range(naux, r, N) of the
+    # auxiliary index, builds its partial J, K over it and the ranks all-reduce the contiguous [J; K]
+    # inside the timed region (strong scaling; PAPER.md:157 q partition, PAPER.md:53 K is a
+    # sum over q).  From here on `naux` is this rank's share; cfg.naux stays the whole build's.
+    q0, q1 = sharded.shard_range(cfg.naux, rank, world)
+    naux = q1 - q0
+    if any(b == a for a, b in (sharded.shard_range(cfg.naux, r, world) for r in range(world))):
+        # every rank takes this branch together (the partition is a pure function of naux and N)
+        raise SystemExit(f"{cfg.naux} auxiliary functions in 512-q blocks leave a rank of {world} without work: "
+                         f"use at most {(cfg.naux + 511) // 512} GPUs for this config")
+    cfg_rank = dataclasses.replace(cfg, naux=naux)  # what this rank's kernels process (roofline numerators)
     B = G.make_B_packed_torch(nao, naux, cfg.seed + rank, device=dev, offdiag_decay=args.screen)
     C0 = G.make_C_occ(nao, nocc, cfg.seed)
     D0 = G.make_density(C0)
@@ -354,8 +366,7 @@ def run_ours(args, cfg):
     D_pin = [torch.from_numpy(Dk).pin_memory() for _, Dk, _ in seq]
     C_pin = [torch.from_numpy(Ck).pin_memory() for _, _, Ck in seq]
     D_buf, C_buf = torch.empty_like(D_dev[0]), torch.empty_like(C_dev[0])
-    J = torch.empty((nao, nao), dtype=torch.float64, device=dev)
-    K = torch.empty_like(J)
+    _JK, J, K = sharded.alloc_jk(nao, dev)  # adjacent halves of one buffer: one all-reduce per build
     J_pin, K_pin = torch.empty((nao, nao), dtype=torch.float64).pin_memory(), torch.empty((nao, nao), dtype=torch.float64).pin_memory()
 
     # ---- workspace: as many 512-q blocks per launch as fit beside B
@@ -487,9 +498,9 @@ def run_ours(args, cfg):
         ms_planned_e2e = timed(args.steps, False, args.warmup)
         same = bool(torch.equal(J, J_ref)) and bool(torch.equal(K, K_ref))
         assert p.df_last_status() == 0
-        planned = {"value": args.steps * world / (ms_planned / 1e3), "unit": UNIT,
+        planned = {"value": args.steps / (ms_planned / 1e3), "unit": UNIT,
                    "ms_per_step": ms_planned / args.steps,
-                   "e2e_value": args.steps * world / (ms_planned_e2e / 1e3),
+                   "e2e_value": args.steps / (ms_planned_e2e / 1e3),
                    "plan_create_ms": pe0.elapsed_time(pe1), "plan_gb": plan_bytes / 1e9, "plan_slices": smax,
                    "bit_identical_to_unplanned": same,
                    "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof_planned.items() if v[1]},
@@ -503,12 +514,12 @@ def run_ours(args, cfg):
             dist.destroy_process_group()
         return
 
-    units = args.steps * world  # shard-builds of this config processed by all ranks
+    units = args.steps  # builds of the config's whole problem, whatever the number of ranks
     value = units / (ms_total / 1e3)
     e2e_value = units / (ms_e2e / 1e3)
     used = [slices[i % nseq] for i in range(args.warmup, args.warmup + args.steps)]
-    ops5 = sum(int8_ops_per_build(cfg, s)[0] for s in used)
-    ops6 = sum(int8_ops_per_build(cfg, s)[1] for s in used)
+    ops5 = sum(int8_ops_per_build(cfg_rank, s)[0] for s in used)  # rank 0's kernels: its own q-shard
+    ops6 = sum(int8_ops_per_build(cfg_rank, s)[1] for s in used)
     ms5, n5 = prof["gemm5_i8"]
     ms6, n6 = prof["gemm6_i8"]
     msu, nu = prof["jk_unpack_split"]
@@ -524,8 +535,8 @@ def run_ours(args, cfg):
     # tensor-pipe-active percentages are the clock-independent one.
     peak_tops = 2.0 * peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
     achieved = (ops5 + ops6) / ((ms5 + ms6) / 1e3) / 1e12
-    ubytes = sum(unpack_bytes_per_build(cfg, s) for s in used)
-    ubytes_design = sum(unpack_bytes_per_build(cfg, s, design=True) for s in used)
+    ubytes = sum(unpack_bytes_per_build(cfg_rank, s) for s in used)
+    ubytes_design = sum(unpack_bytes_per_build(cfg_rank, s, design=True) for s in used)
     hbm_achieved = ubytes / (msu / 1e3) / 1e9 if msu else None
 
     def pipe_pct(cls):
@@ -549,9 +560,11 @@ def run_ours(args, cfg):
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "int8", "dtype_note": "int8 x int8 -> int32 slice-pair products, f64 recombination; J in f64",
+        "scaling": "weak" if world == 1 else "strong", "vs_baseline": None, "dtype": "int8", "dtype_note": "int8 x int8 -> int32 slice-pair products, f64 recombination; J in f64",
         "data": "synthetic",
-        "config": {"workload": workload_name(args.config, cfg) + (", 12-step adaptive SCF sequence" if nseq == NSEQ else ", tol alternating 1e-6 / 1e-10") + ", one q-shard per GPU",
+        "config": {"workload": workload_name(args.config, cfg) + (", 12-step adaptive SCF sequence" if nseq == NSEQ else ", tol alternating 1e-6 / 1e-10")
+                               + (f", q-sharded over {world} GPUs (512-aligned ranges, one all-reduce of [J; K] per build)" if world > 1 else ""),
+                   "q_shard_rank0": [q0, q1],
                    "slices_per_step": used, "tol_per_step": [tols[i % nseq] for i in range(args.warmup, args.warmup + args.steps)],
                    "l2": "inputs larger than L2: packed B is %.1f GB and every step streams it" % (B.numel() * 8 / 1e9),
                    "screen_decay": args.screen,
@@ -715,16 +728,7 @@ def run_gemm(args):
         if n <= 4096:
             A, B = (torch.from_numpy(x).to(dev) for x in G.make_gemm_inputs(n, n, n, seed=n))
         else:  # same distribution (R10), generated on the device
-            g = torch.Generator(device=dev)
-            g.manual_seed(n)
-
-            def one():
-                e = torch.rand((n, n), generator=g, dtype=torch.float64, device=dev) * 30.0 - 30.0
-                off = torch.randint(-10, 11, (n, 1), generator=g, device=dev).to(torch.float64)
-                sgn = torch.where(torch.rand((n, n), generator=g, device=dev) < 0.5, -1.0, 1.0).to(torch.float64)
-                return sgn * torch.exp2(e + off)
-
-            A, B = one(), one()
+            A, B = G.make_gemm_inputs_torch(n, n, n, seed=n, device=dev)
         C = torch.empty((n, n), dtype=torch.float64, device=dev)
         ref = A @ B
         torch.matmul(A, B, out=ref)
@@ -792,6 +796,24 @@ def main():
         distill_ncu_raw(args.ncu_raw)
         return
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started by hand without a launcher: start the N ranks ourselves (the driver starts them with
+        # torch.distributed.run; this is the same command line)
+        if args.impl == "ours":
+            import torch
+
+            have = torch.cuda.device_count()
+            if have < args.gpus:
+                sys.stderr.write(f"bench.py --gpus {args.gpus}: this node has {have} CUDA device(s); one rank per GPU, "
+                                 "no oversubscription (ranks that wait on one another cannot share a GPU)\n")
+                raise SystemExit(2)
+        from paper_2601_08077_b200.sharded import launcher_command
+
+        cmd = launcher_command(args.gpus, os.path.abspath(__file__), sys.argv[1:])
+        os.execv(cmd[0], cmd)
+    if "WORLD_SIZE" in os.environ and int(os.environ["WORLD_SIZE"]) != args.gpus and args.impl == "ours":
+        sys.stderr.write(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={os.environ['WORLD_SIZE']}\n")
+        raise SystemExit(2)
     if args.config == "gemm":
         if args.impl == "reference":
             print(json.dumps({"impl": "reference", "unavailable": "the reference arm is defined for the DF J/K configs"}))

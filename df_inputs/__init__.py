@@ -17,6 +17,7 @@ from .generators import (  # noqa: F401
     make_density,
     make_df_inputs,
     make_gemm_inputs,
+    make_gemm_inputs_torch,
     make_scf_sequence,
     occ_from_density,
     make_B_packed_torch,

@@ -112,6 +112,24 @@ def make_gemm_inputs(m: int, n: int, k: int, seed: int):
     return one(m, k), one(k, n)
 
 
+def make_gemm_inputs_torch(m: int, n: int, k: int, seed: int, device="cuda"):
+    """make_gemm_inputs generated on the device for the sizes too large for host time (8192, 16384):
+    the same distribution (sign 2^e, real e ~ Uniform(-30, 0), integer per-row offsets in [-10, 10]),
+    NOT the same bytes -- a consumer on the host reads these bytes back, it never regenerates them."""
+    import torch
+
+    g = torch.Generator(device=device)
+    g.manual_seed(seed)
+
+    def one(rows, cols):
+        e = torch.rand((rows, cols), generator=g, dtype=torch.float64, device=device) * 30.0 - 30.0
+        off = torch.randint(-10, 11, (rows, 1), generator=g, device=device).to(torch.float64)
+        sgn = torch.where(torch.rand((rows, cols), generator=g, device=device) < 0.5, -1.0, 1.0).to(torch.float64)
+        return sgn * torch.exp2(e + off)
+
+    return one(m, k), one(k, n)
+
+
 def occ_from_density(D: np.ndarray, nocc: int) -> np.ndarray:
     """C with D ~= 2 C C^T from the nocc largest eigenpairs."""
     lam, V = np.linalg.eigh(0.5 * (D + D.T))

@@ -18,6 +18,19 @@ def dev(x):
     return torch.from_numpy(np.ascontiguousarray(x)).to(DEV)
 
 
+def assert_k_matches_emulation(K, K_emu):
+    """K of the CUDA path against the oracle's emulated K.  X and every GEMM(6) scale index are
+    bit-equal, so the two differ only in the order of the FP64 additions over the q-groups (SURVEY.md
+    8(c): a tolerance for the last bits): 1e-14 in the Frobenius norm, and no single entry off by more
+    than 1e-13 of its Cauchy-Schwarz scale sqrt(K_ii K_jj) -- a norm alone would hide one wrong entry."""
+    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    d = np.sqrt(np.maximum(np.diag(K_emu), 0.0))
+    scale = np.outer(d, d)
+    diff = np.abs(K - K_emu)
+    assert not diff[scale == 0.0].any()
+    assert np.max(diff[scale > 0.0] / scale[scale > 0.0], initial=0.0) <= 1e-13
+
+
 def edge_matrix(rows, cols, seed):
     """Random wide-range rows plus the scale-index edge cases of DESIGN.md R2."""
     rng = np.random.default_rng(seed)
@@ -215,7 +228,7 @@ def test_jk_tiny_config0(dfe, gpu_ws, tol):
     for g, (g0, g1) in enumerate(groups):
         Xrow = np.transpose(X_emu[g0:g1], (1, 0, 2)).reshape(cfg.nao, -1)
         assert np.array_equal(e6[g], O.scale_index(np.max(np.abs(Xrow), axis=1)))
-    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert_k_matches_emulation(K, K_emu)
     assert np.array_equal(J, J.T) and np.array_equal(K, K.T)
     assert np.linalg.eigvalsh(K).min() >= -1e-12 * np.abs(K).max()
     assert dfe.df_last_status() == 0
@@ -243,7 +256,7 @@ def test_jk_many_groups_and_superblocks(dfe, gpu_ws):
     for g, (g0, g1) in enumerate(groups):
         Xrow = np.transpose(X_emu[g0:g1], (1, 0, 2)).reshape(nao, -1)
         assert np.array_equal(e6[g], O.scale_index(np.max(np.abs(Xrow), axis=1)))
-    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert_k_matches_emulation(K, K_emu)
     assert O.rel_frobenius(K, K_ref) <= 1e-12 and O.rel_frobenius(J, J_ref) <= 1e-12
     small = dfe.Workspace(dfe.df_jk_workspace_bytes(nao, naux, nocc, s))
     try:
@@ -275,7 +288,7 @@ def test_jk_group_boundaries_off_32(dfe, gpu_ws, nocc, s, naux):
     for g, (g0, g1) in enumerate(groups):
         Xrow = np.transpose(X_emu[g0:g1], (1, 0, 2)).reshape(nao, -1)
         assert np.array_equal(e6[g], O.scale_index(np.max(np.abs(Xrow), axis=1)))
-    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert_k_matches_emulation(K, K_emu)
     assert np.array_equal(K, K.T) and dfe.df_last_status() == 0
 
 
@@ -294,7 +307,7 @@ def test_jk_split_n_tiles(dfe, gpu_ws, s):
     J_ref, K_ref = O.df_jk_plain(Bp, nao, Cocc, D)
     assert np.array_equal(X[:, :, :nocc], X_emu)
     assert not X[:, :, nocc:].any()
-    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert_k_matches_emulation(K, K_emu)
     assert O.rel_frobenius(J, J_ref) <= 1e-12
     assert O.rel_frobenius(K, K_ref) <= {4: 1e-6, 5: 1e-9, 6: 1e-11, 8: 1e-12}[s]  # 2^(8 - 8 s) and margin
     assert dfe.df_last_status() == 0
@@ -314,7 +327,7 @@ def test_jk_every_slice_count_ragged(dfe, gpu_ws, s):
     J_ref, _ = O.df_jk_plain(Bp, nao, Cocc, D)
     assert np.array_equal(X[:, :, :nocc], X_emu)
     assert not X[:, :, nocc:].any()
-    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert_k_matches_emulation(K, K_emu)
     assert O.rel_frobenius(J, J_ref) <= 1e-12
     assert np.array_equal(K, K.T) and dfe.df_last_status() == 0
 
@@ -342,7 +355,7 @@ def test_jk_planned_build_bitwise(dfe, gpu_ws, smax):
         torch.cuda.synchronize()
         assert torch.equal(J, J2) and torch.equal(K, K2), s
         K_emu = O.emul_df_k(Bp, nao, Cocc, s)
-        assert O.rel_frobenius(K2.cpu().numpy(), K_emu) <= 1e-14
+        assert_k_matches_emulation(K2.cpu().numpy(), K_emu)
     # tol entry point: same policy as df_jk_build
     tol = 1e-6
     dfe.df_jk_build(Bd, nao, naux, dev(Cocc), nocc, dev(D), tol, J, K)
@@ -432,15 +445,41 @@ def test_jk_medium_config2(dfe, gpu_ws):
     assert dfe.df_last_status() == 0
 
 
+_CONFIG4_REF = {}  # the oracle's J (all q) and K (first 512 q) of config 4, computed once per session
+
+
+def config4_oracle_refs(B, cfg, Cocc, D, qs):
+    """The oracle's plain FP64 J over all of config 4 (rho_q and J are sums over q, Eqs. 3-4: the 78 GB
+    of device bytes are streamed to the host in 512-q blocks, about a minute) and its K over the first
+    `qs` auxiliary functions (Eq. 6; K over all 6000 would take ten minutes)."""
+    if not _CONFIG4_REF:
+        nao, naux = cfg.nao, cfg.naux
+        rho = np.empty(naux)
+        J_ref = np.zeros((nao, nao))
+        K_ref = None
+        for q0 in range(0, naux, 512):
+            q1 = min(naux, q0 + 512)
+            Bb = B[:, q0:q1].contiguous().cpu().numpy()
+            rho[q0:q1] = O.df_rho(Bb, nao, D)
+            J_ref += O.df_j(Bb, nao, rho[q0:q1])
+            if q0 == 0:
+                K_ref = O.df_k(Bb[:, :qs], nao, Cocc)
+            del Bb
+        _CONFIG4_REF.update(J_ref=J_ref, K_ref=K_ref, rho=rho)
+    return _CONFIG4_REF
+
+
 @pytest.mark.parametrize("tol", [1e-6, 1e-10])
 def test_jk_largest_config4(dfe, gpu_ws, tol):
     """BASELINE.json config 4 at full size (nao 1800, naux 6000, nocc 250; packed B 78 GB on the
     device, naux processed in super-blocks of two 512-q blocks) at both tolerances it names
     (s = 4: GEMM(5) as two 128-column N tiles on MMA pairs; s = 6: on multicast CTA pairs with a
     second pass).  X of sampled q bit for bit against the oracle's emulation of GEMM(5) from the same
-    bytes, every GEMM(6) scale index exactly, sampled K entries against the oracle's definition within
-    tol, symmetry and the trace invariant.  (The plain FP64 oracle over all 6000 q of this size takes
-    ~10 minutes of host time: the full-matrix comparison is the config-3 test.)"""
+    bytes, every GEMM(6) scale index exactly, J as a FULL matrix against the oracle's plain FP64 J of the
+    same bytes (<= 1e-12), K as a full matrix on a 512-q sub-build (the shape of bench.py's parity
+    check) against the oracle's K within tol, norm and element-wise, sampled entries of the full-size K
+    against the oracle's definition, symmetry and the trace invariants.  (The oracle's K over all 6000 q
+    of this size takes ~10 minutes of host time: the full-size full-matrix K comparison is the config-3 test.)"""
     torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 140 << 30:
@@ -480,12 +519,30 @@ def test_jk_largest_config4(dfe, gpu_ws, tol):
             m = X[g0:g1].abs().amax(dim=(0, 2)).cpu().numpy()
             assert np.array_equal(e6h[g], O.scale_index(m)), f"group {g}"
         del X, J2, K2
+        # the first 512 q as a build of their own: K as a full matrix against the oracle
+        qs = 512
+        ref = config4_oracle_refs(B, cfg, Cocc, D, qs)
+        Bs = B[:, :qs].contiguous()
+        Js, Ks = torch.empty_like(J), torch.empty_like(K)
+        dfe.df_jk_build(Bs, nao, qs, dev(Cocc), nocc, dev(D), tol, Js, Ks)
+        torch.cuda.synchronize()
+        Ksh = Ks.cpu().numpy()
+        del Bs, Js, Ks
+        eKs = O.rel_frobenius(Ksh, ref["K_ref"])
+        assert eKs <= tol, (eKs, tol, s)
+        dK = np.sqrt(np.diag(ref["K_ref"]))
+        assert np.max(np.abs(Ksh - ref["K_ref"]) / np.outer(dK, dK)) <= tol
     finally:
         big.close()
         dfe.df_set_workspace(gpu_ws.view)
     Jh, Kh = J.cpu().numpy(), K.cpu().numpy()
     assert np.array_equal(Jh, Jh.T) and np.array_equal(Kh, Kh.T)
     assert np.isfinite(Jh).all() and np.isfinite(Kh).all()
+    # J over all 6000 q, full matrix (J is plain FP64 on both sides: PAPER.md:101)
+    eJ = O.rel_frobenius(Jh, ref["J_ref"])
+    assert eJ <= 1e-12, eJ
+    rho = ref["rho"]
+    assert abs(np.sum(D * Jh) - rho @ rho) <= 1e-11 * (rho @ rho)  # Tr(D J) = |rho|^2
 
     def x_rows(i):  # X_i[q, a] = sum_j B^q_ij C_ja from the packed rows of i (Eq. 5)
         idx = torch.tensor([max(i, j) * (max(i, j) + 1) // 2 + min(i, j) for j in range(nao)], device=DEV)
@@ -496,7 +553,6 @@ def test_jk_largest_config4(dfe, gpu_ws, tol):
             kij = float(np.sum(rows[i] * rows[j]))  # Eq. 6
             scale = np.sqrt(np.sum(rows[i] ** 2) * np.sum(rows[j] ** 2))
             assert abs(Kh[i, j] - kij) <= tol * scale, (i, j, Kh[i, j], kij)
-    # J needs all of rho (78 GB streamed to the host): its full-size check is the config-3 test
     assert np.sum(D * Kh) >= 0.0
     del B
 
@@ -616,7 +672,7 @@ def test_jk_nocc_250_like(dfe, gpu_ws, s):
     J_ref, K_ref = O.df_jk_plain(Bp, nao, Cocc, D)
     assert np.array_equal(X[:, :, :nocc], X_emu)
     assert not X[:, :, nocc:].any()
-    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert_k_matches_emulation(K, K_emu)
     assert O.rel_frobenius(J, J_ref) <= 1e-12
     assert O.rel_frobenius(K, K_ref) <= (1e-6 if s == 4 else 1e-10)
     assert np.array_equal(K, K.T)
@@ -641,6 +697,39 @@ def test_emul_gemm_4096_sampled_rows_bitwise(dfe, gpu_ws, s):
     err = O.rel_frobenius(Cg[rows], O.gemm_plain(A[rows], B))
     assert err <= (1e-6 if s == 4 else 1e-12), err
     assert dfe.df_last_status() == 0
+
+
+@pytest.mark.parametrize("s", [4, 8])
+def test_emul_gemm_16384_sampled_tiles_bitwise(dfe, gpu_ws, s):
+    """the bit-exact integer check at the FULL size of BASELINE.json configs[1],
+    16384^3, in the launch configuration bench.py --config gemm times.  At s = 8 the contraction exceeds
+    KFLUSH(8) = 16352: the launch takes a second flush chunk of 32 elements on cta_group::2 pair tiles
+    (the global read-modify-write of the running sum).  The operands are generated on the device
+    (same distribution as make_gemm_inputs) and read back; the oracle emulates sampled rows of A against
+    sampled columns of B over the full K -- first / last / boundary 128-tiles -- and those entries of C
+    must match bit for bit."""
+    n = 16384
+    if s == 8:
+        assert dfe.df_kflush(8) == 16352 < n
+    if dfe.df_emul_gemm_workspace_bytes(n, n, n, s) > gpu_ws.view.numel():
+        pytest.skip("workspace fixture too small")
+    A, B = G.make_gemm_inputs_torch(n, n, n, seed=77, device=DEV)
+    C = torch.empty((n, n), dtype=torch.float64, device=DEV)
+    dfe.df_emul_gemm_slices(A, B, C, n, n, n, s)
+    torch.cuda.synchronize()
+    assert dfe.df_last_status() == 0
+    rows = np.array([0, 1, 127, 128, 255, 256, 8191, 8192, 12345, 16383])
+    cols = np.concatenate([np.arange(0, 130), np.arange(8190, 8194), np.arange(16384 - 130, 16384), [4099, 11111]])
+    ti, tj = torch.from_numpy(rows).to(DEV), torch.from_numpy(cols).to(DEV)
+    Ah = A.index_select(0, ti).cpu().numpy()                      # sampled rows of A, all of K
+    Bh = B.index_select(1, tj).cpu().numpy()                      # all of K, sampled columns of B
+    got = C.index_select(0, ti).index_select(1, tj).cpu().numpy()
+    eA, DA = O.split_operand(Ah, s)
+    eB, DB = O.split_operand(np.ascontiguousarray(Bh.T), s)       # one scale per column of B
+    assert np.array_equal(got, O.emul_gemm_digits(eA, DA, eB, DB, s))
+    err = O.rel_frobenius(got, O.gemm_plain(Ah, Bh))
+    assert err <= (1e-6 if s == 4 else 1e-12), err
+    del A, B, C
 
 
 @pytest.mark.parametrize("flags", [8, 1 << 20, (1 << 20) | 8, 32 << 8, 64 << 8, 128 << 8, 1 << 23, (1 << 23) | 8, 1 << 24])
@@ -677,7 +766,7 @@ def test_jk_alternative_gemm5_paths(dfe, gpu_ws, flags):
             J, K, X, e6, ng = run_jk(dfe, Bp, nao, naux, Cocc, nocc, D, s)
             K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
             assert np.array_equal(X[:, :, :nocc], X_emu), f"s={s}"
-            assert O.rel_frobenius(K, K_emu) <= 1e-14
+            assert_k_matches_emulation(K, K_emu)
     finally:
         dfe.lib.df_debug_set_gemm_flags(0)
 
@@ -886,7 +975,7 @@ def test_jk_screened_input_bit_exact(dfe, gpu_ws, s):
     for g, (g0, g1) in enumerate(groups):
         Xrow = np.transpose(X_emu[g0:g1], (1, 0, 2)).reshape(nao, -1)
         assert np.array_equal(e6[g], O.scale_index(np.max(np.abs(Xrow), axis=1)))
-    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert_k_matches_emulation(K, K_emu)
     assert O.rel_frobenius(J, J_ref) <= 1e-12
     assert dfe.df_last_status() == 0
     # screening off: every block is written, loaded and multiplied -- the same bits
@@ -935,7 +1024,7 @@ def test_jk_screened_wide_mask_and_superblocks(dfe, gpu_ws):
     assert total == ((naux * nao + 255) // 256) * 33 and 0 < active < 0.6 * total, (active, total)
     K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
     assert np.array_equal(X[:, :, :nocc], X_emu)
-    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert_k_matches_emulation(K, K_emu)
     del Bp, X, X_emu
 
     nao, naux, nocc, s = 300, 1100, 12, 4
@@ -953,7 +1042,7 @@ def test_jk_screened_wide_mask_and_superblocks(dfe, gpu_ws):
     assert 0 < active < total
     K_emu, X_emu = O.emul_df_k(Bp, nao, Cocc, s, return_x=True)
     assert np.array_equal(X[:, :, :nocc], X_emu)
-    assert O.rel_frobenius(K, K_emu) <= 1e-14
+    assert_k_matches_emulation(K, K_emu)
     J_ref, _ = O.df_jk_plain(Bp, nao, Cocc, D)
     assert O.rel_frobenius(J, J_ref) <= 1e-12
 

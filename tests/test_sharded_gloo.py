@@ -43,11 +43,17 @@ def _worker(rank, world, port, out):
     q0, q1 = sharded.shard_range(naux, rank, world)
     Bs = np.ascontiguousarray(Bp[:, q0:q1])
     Jp, Kp = O.emul_df_jk(Bs, nao, Cocc, D, s)
-    J, K = torch.from_numpy(Jp.copy()), torch.from_numpy(Kp.copy())
+    _JK, J, K = sharded.alloc_jk(nao)  # adjacent halves of one buffer: the exchange is ONE all-reduce
+    J.copy_(torch.from_numpy(Jp))
+    K.copy_(torch.from_numpy(Kp))
+    calls = []
+    real = dist.all_reduce
+    dist.all_reduce = lambda t, *a, **kw: (calls.append(t.numel()), real(t, *a, **kw))[1]
     sharded.allreduce_jk(J, K)
+    dist.all_reduce = real
     if rank == 0:
         Jf, Kf = O.emul_df_jk(Bp, nao, Cocc, D, s)
-        out.put((O.rel_frobenius(J.numpy(), Jf), O.rel_frobenius(K.numpy(), Kf)))
+        out.put((O.rel_frobenius(J.numpy(), Jf), O.rel_frobenius(K.numpy(), Kf), calls))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -128,9 +134,44 @@ def test_two_rank_allreduce_equals_single_build():
     procs = [ctx.Process(target=_worker, args=(r, 2, port, out)) for r in range(2)]
     for p in procs:
         p.start()
-    eJ, eK = out.get(timeout=240)
+    eJ, eK, calls = out.get(timeout=240)
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
     # same q-groups (shards are multiples of 512), only the FP64 summation order differs
     assert eJ <= 1e-14 and eK <= 1e-14
+    assert calls == [2 * 24 * 24]  # one all-reduce over the contiguous [J; K]
+
+
+def _bench(*argv):
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    return subprocess.run([sys.executable, os.path.join(root, "bench.py"), *argv], capture_output=True, text=True,
+                          env=env, timeout=600)
+
+
+def test_bench_gpus_2_starts_two_ranks_through_the_launcher():
+    """`bench.py --gpus 2` started by hand (no WORLD_SIZE) re-executes itself under
+    sharded.launcher_command -- torch.distributed.run, rendezvous on 127.0.0.1 -- as two ranks.  Driven
+    here with the CPU arm (the oracle; no GPU needed): rank 0 prints the one JSON line, rank 1 exits 0."""
+    import json
+
+    r = _bench("--gpus", "2", "--impl", "reference", "--config", "tiny", "--steps", "1", "--warmup", "0", "--ref-q", "16")
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
+
+
+def test_bench_gpus_beyond_the_devices_fails_loudly():
+    """The product arm never oversubscribes a GPU: more ranks than devices is an error, not n_gpus = 1."""
+    import torch
+
+    n = torch.cuda.device_count() + 1 if torch.cuda.is_available() else 2
+    r = _bench("--gpus", str(max(2, n)), "--config", "tiny", "--steps", "1")
+    assert r.returncode == 2
+    assert "CUDA device" in r.stderr and not [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
