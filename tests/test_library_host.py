@@ -247,3 +247,31 @@ def test_measured_density_changes_of_the_synthetic_sequence():
         assert 0.8 * want <= dD[k] <= 1.25 * want, (k, dD[k], want)
     levels = [lv for lv, _ in policy.schedule_from_density_change(dD)][:12]
     assert levels[0] == levels[1] == 4 and all(a >= b for a, b in zip(levels[:-1], levels[1:]))
+
+
+def test_ncu_table_is_rederivable_and_detects_stale_sources(tmp_path, monkeypatch):
+    """profiles/ncu_kernels.csv (the counters bench.py quotes as roofline.traffic and tensor-pipe %) is
+    what `bench.py --ncu-raw` distils from the committed raw ncu export, row for row; and the table is
+    dropped (traffic null, traffic_stale true) as soon as the kernel sources differ from the ones it
+    was captured on."""
+    import csv
+    import sys
+
+    sys.path.insert(0, ROOT)
+    import bench
+
+    raw = os.path.join(ROOT, "profiles", "r03_ncu_full_raw.csv")
+    committed = list(csv.DictReader(open(os.path.join(ROOT, bench.NCU_TABLE))))
+    assert {(r["kernel_class"], r["s"]) for r in committed} >= {(c, str(s)) for c in ("gemm5_i8", "gemm6_i8", "jk_unpack_split")
+                                                               for s in (4, 5, 6)}
+    monkeypatch.setattr(bench, "NCU_TABLE", str(tmp_path / "t.csv"))
+    bench.distill_ncu_raw([raw])
+    again = list(csv.DictReader(open(tmp_path / "t.csv")))
+    strip = lambda rows: [{k: v for k, v in r.items() if k != "sources_sha16"} for r in rows]
+    assert strip(again) == strip(committed)
+    table, stale = bench.ncu_table()
+    assert not stale and len(table) == len(committed)  # distilled just now from these sources
+    monkeypatch.setattr(bench, "kernel_sources_sha16", lambda: "0" * 16)
+    table, stale = bench.ncu_table()
+    assert stale
+    assert bench.traffic_for_mix({}, ("gemm5_i8", "gemm6_i8"), [4, 5]) is None
